@@ -1,0 +1,137 @@
+/* mspcg.h -- C ABI of libmspcg: the single-GPU (B200, sm_100a) hot path of multi-splitting preconditioned CG
+ * (MSPCG) for the even-odd preconditioned Moebius domain-wall normal equations  D^dag D x = b.
+ *
+ * Paper: arXiv 2104.05615 (PAPER.md in the reference mount).  Citations below are PAPER.md line numbers plus the
+ * section / equation; "R<n>" are the readings of silent or garbled passages listed in DESIGN.md.
+ *
+ * Plain C, plain pointers and sizes.  Every pointer says whether it is HOST or DEVICE memory.  The library never
+ * allocates device memory for vectors, tables or link copies: the caller (PyTorch, in this repository) owns one
+ * workspace buffer and every input / output buffer.  All calls return an mspcg status (0 = OK, negative = error),
+ * never throw and never exit; mspcg_last_error() gives a message for the last failing call on that context.
+ *
+ * ---------------------------------------------------------------------------------------------------------------
+ * Vector layouts
+ *
+ *  ABI layout (fp64 only): even-parity 5D spinor  psi[s][x_cb][spin 4][colour 3][re,im],  x_cb = lex/2 over even
+ *      sites, lex = x + Lx*(y + Ly*(z + Lz*t)), parity = (x+y+z+t) mod 2 (eq. 3).  Spin index in the
+ *      chiral basis of R2 (gamma5 = diag(+,+,-,-)).  Ls*V4/2*24 doubles.
+ *  NATIVE layout (precision prec): the library's private site-slab layout, mspcg_vec_bytes(ctx, prec) bytes; made by
+ *      mspcg_pack and read back by mspcg_unpack.  Operator calls on NATIVE vectors do no layout conversion.
+ *  Gauge ABI layout: U[mu][parity][x_cb][row 3][col 3][re,im] fp64, mu = 0..3 <-> x,y,z,t, periodic links (the
+ *      antiperiodic time boundary is requested with t_boundary = -1 and folded in by the library, R7).
+ * --------------------------------------------------------------------------------------------------------------- */
+#ifndef MSPCG_H
+#define MSPCG_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mspcg_ctx mspcg_ctx; /* opaque, library-owned (host memory) */
+
+enum { MSPCG_OK = 0, MSPCG_EINVAL = -1, MSPCG_ENOMEM = -2, MSPCG_ECUDA = -3, MSPCG_ENOGAUGE = -4,
+       MSPCG_ENOCONV = -5, MSPCG_EBREAKDOWN = -6, MSPCG_ENOWORKSPACE = -7 };
+enum { MSPCG_F64 = 8, MSPCG_F32 = 4, MSPCG_F16 = 2 };   /* storage precision of vectors and link copies       */
+enum { MSPCG_LAYOUT_ABI = 0, MSPCG_LAYOUT_NATIVE = 1 }; /* layout of the in/out buffers of the apply calls    */
+
+/* Create a context: lattice Lx,Ly,Lz,Lt (all even), fifth dimension Ls, Moebius parameters b, c, M5 (domain-wall
+ * height) and mf (eq. 4-8; operator entries: R1-R4), and the Dirichlet block ("virtual node",
+ * PAPER.md:162-176 eq. 12-14) extents Bx..Bt: every B even, dividing L; B == L means that direction is not cut.
+ * HOST-only work (index tables, Ls x Ls matrices): needs no GPU.  Errors: MSPCG_EINVAL for odd L or B, L % B != 0,
+ * Ls < 2 or not one of the compiled values {4,6,8,12,16}, alpha = b(4-M5)+1 == 0. */
+int mspcg_create(mspcg_ctx** out, int Lx, int Ly, int Lz, int Lt, int Ls, double b, double c, double M5, double mf,
+                 int Bx, int By, int Bz, int Bt);
+int mspcg_destroy(mspcg_ctx* ctx);
+const char* mspcg_last_error(const mspcg_ctx* ctx);
+
+/* Host-side geometry facts (no GPU): out[0]=number of blocks, out[1]=4D sites of one parity inside a block (E0),
+ * out[2]=even 4D sites with L1 overshoot <= 2 (E2), out[3]=odd 4D sites with overshoot <= 1 (O1)
+ * (minimal site sets of PAPER.md:226, R11), out[4]=V4/2. */
+int mspcg_geometry(const mspcg_ctx* ctx, long out[5]);
+/* The P+ chirality block (Ls x Ls, row major, HOST) of which = 0: M5, 1: Mphi, 2: M5^-1 (R3, R4). */
+int mspcg_get_matrix(const mspcg_ctx* ctx, int which, double* out_host);
+
+/* Precisions this context will run in, and the workspace they need.  outer_prec: the sloppy precision of the outer
+ * iteration and of mspcg_apply_MdagM besides fp64 (fp64 is always available); inner_prec: storage precision of the
+ * preconditioner (R14); recon: 18, or 12 = two-row link storage with the third row rebuilt in the
+ * kernels (R8) for the non-fp64 link copies.  Returns the byte count through *bytes. */
+int mspcg_workspace_bytes(mspcg_ctx* ctx, int outer_prec, int inner_prec, int recon, size_t* bytes);
+/* Hand the library its workspace (DEVICE, 256-byte aligned, >= the size above; caller keeps ownership and must keep
+ * it alive until mspcg_destroy).  Uploads the index tables on `stream` (a cudaStream_t passed as void*). */
+int mspcg_set_workspace(mspcg_ctx* ctx, void* workspace_dev, size_t bytes, void* stream);
+
+/* Ingest a gauge field: U_dev is DEVICE fp64 in the gauge ABI layout (4*V4*18
+ * doubles).  t_boundary = +1 periodic / -1 antiperiodic in time (R7).  Builds the per-stage link copies in every
+ * configured precision.  Asynchronous on `stream`. */
+int mspcg_load_gauge(mspcg_ctx* ctx, const double* U_dev, int t_boundary, void* stream);
+
+/* NATIVE <-> ABI conversion of even-parity vectors (DEVICE pointers, asynchronous). */
+size_t mspcg_vec_bytes(const mspcg_ctx* ctx, int prec);
+int mspcg_pack(mspcg_ctx* ctx, const double* abi_dev, void* native_dev, int prec, void* stream);
+int mspcg_unpack(mspcg_ctx* ctx, const void* native_dev, double* abi_dev, int prec, void* stream);
+
+/* out = D^dag D in  on the whole periodic/antiperiodic lattice (eq. 9-10, 230-258 eq. 15-16:
+ * one Mphi kernel and four fused hop kernels).  prec = MSPCG_F64 or the configured outer_prec.
+ * layout ABI: in/out are fp64 ABI vectors (converted on entry/exit); NATIVE: vectors of `prec` from mspcg_pack.
+ * in and out must not alias.  Asynchronous on `stream`.  Errors: ENOGAUGE, ENOWORKSPACE, EINVAL. */
+int mspcg_apply_MdagM(mspcg_ctx* ctx, const void* in_dev, void* out_dev, int prec, int layout, void* stream);
+
+/* z = M^-1 r: the multi-splitting preconditioner (eq. 12-14): for every Dirichlet block
+ * independently, n_inner CG iterations from a zero guess (R13) on A_s z_s = r_s, A_s being the block's
+ * part of D^dag D including the snake terms (eq. 11, 224-228; R10 reading PAD).  All blocks run
+ * batched in the same launches.  io_prec: precision of r and z (F64 or outer_prec); the inner iteration runs in the
+ * configured inner_prec (fp16 storage: per-block max-abs scaling, fp32 arithmetic).  If a reduced-Ls transfer
+ * matrix is set and use_reduced != 0:  z = T^dag CG_k[M-hat](T r) + mu r (eq. 19-21). */
+int mspcg_apply_precond(mspcg_ctx* ctx, const void* r_dev, void* z_dev, int io_prec, int layout, int n_inner,
+                        int use_reduced, void* stream);
+/* The same two operator calls on HOST fp64 ABI buffers: host->device copy, apply, device->host copy, synchronous.
+ * (End-to-end path used by bench.py's e2e figure.) */
+int mspcg_apply_MdagM_host(mspcg_ctx* ctx, const double* in_host, double* out_host, int prec);
+int mspcg_apply_precond_host(mspcg_ctx* ctx, const double* r_host, double* z_host, int io_prec, int n_inner,
+                             int use_reduced);
+
+/* A_s applied to the block-`block` part of a vector (debug / parity entry: PAPER.md:224, R10): fp64, ABI layout;
+ * out is zero outside the block. */
+int mspcg_apply_A_block(mspcg_ctx* ctx, const double* in_dev, double* out_dev, int block, int prec, void* stream);
+
+/* Reduced-Ls preconditioner: Ls_hat in the compiled set, T_host[4*Ls_hat][4*Ls][re,im] (HOST,
+ * row (s_hat,spin), column (s,spin); identity in colour and 4D site, eq. 21), shift mu (eq. 20).  Must be called
+ * before mspcg_workspace_bytes. */
+int mspcg_set_reduced_ls(mspcg_ctx* ctx, int Ls_hat, const double* T_host, double mu);
+
+typedef struct {
+  double tol;          /* relative residual |r|/|b| (R15)                                                        */
+  int max_iter;        /* outer iteration cap                                                                    */
+  int use_precond;     /* 0: plain CG (z = r), 1: MSPCG                                                          */
+  int n_inner;         /* inner CG iterations per block                                           */
+  int sloppy_prec;     /* MSPCG_F64 (no reliable updates needed) or the configured outer_prec                    */
+  double delta;        /* reliable-update threshold (R17), e.g. 0.1                                              */
+  int use_reduced_ls;  /* 0/1                                                                                    */
+  int history_len;     /* entries available in `history` (HOST) or 0                                             */
+  double* history;     /* HOST: |r_k|/|b| of the iterated residual for k = 1..                                   */
+} mspcg_solve_params;
+
+typedef struct {
+  int iters, reliable_updates, converged, breakdown;
+  long inner_applies;  /* total A_s applications (blocks x inner iterations x outer applications)                */
+  long outer_applies;  /* D^dag D applications, sloppy + precise                                                 */
+  double true_res;     /* |b - A x| / |b| in fp64                                                                */
+  double seconds;      /* device time of the solve, CUDA events                                                  */
+} mspcg_solve_stats;
+
+/* Solve D^dag D x = b (eq. 9) with Algorithm 1 (R15), Polak-Ribiere beta
+ * (eq. 18; R16) and reliable updates (R17).  b_dev, x_dev: DEVICE fp64 ABI vectors;
+ * x_dev holds x0 on entry and the solution on exit.  Synchronous: returns when *stats (HOST) is valid.
+ * Returns MSPCG_OK, MSPCG_ENOCONV (max_iter hit, x = best iterate) or MSPCG_EBREAKDOWN (<p,Ap> <= 0 or NaN). */
+int mspcg_solve(mspcg_ctx* ctx, const double* b_dev, double* x_dev, const mspcg_solve_params* params,
+                mspcg_solve_stats* stats, void* stream);
+
+/* Counters for reports: kernels launched by this context since creation. */
+long mspcg_launch_count(const mspcg_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MSPCG_H */

@@ -1,0 +1,237 @@
+"""Thin ctypes binding of libmspcg (include/mspcg.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI; PyTorch is used here only to own device
+memory (torch tensors) and to name the current CUDA stream.  There is no CPU fallback: if the library is missing
+or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libmspcg.so")
+
+F64, F32, F16 = 8, 4, 2
+LAYOUT_ABI, LAYOUT_NATIVE = 0, 1
+OK, EINVAL, ENOMEM, ECUDA, ENOGAUGE, ENOCONV, EBREAKDOWN, ENOWORKSPACE = 0, -1, -2, -3, -4, -5, -6, -7
+
+SYMBOLS = [
+    "mspcg_create", "mspcg_destroy", "mspcg_last_error", "mspcg_geometry", "mspcg_get_matrix",
+    "mspcg_workspace_bytes", "mspcg_set_workspace", "mspcg_load_gauge", "mspcg_vec_bytes", "mspcg_pack",
+    "mspcg_unpack", "mspcg_apply_MdagM", "mspcg_apply_precond", "mspcg_apply_MdagM_host",
+    "mspcg_apply_precond_host", "mspcg_apply_A_block", "mspcg_set_reduced_ls", "mspcg_solve", "mspcg_launch_count",
+]
+
+
+class SolveParams(C.Structure):
+    _fields_ = [("tol", C.c_double), ("max_iter", C.c_int), ("use_precond", C.c_int), ("n_inner", C.c_int),
+                ("sloppy_prec", C.c_int), ("delta", C.c_double), ("use_reduced_ls", C.c_int),
+                ("history_len", C.c_int), ("history", C.POINTER(C.c_double))]
+
+
+class SolveStats(C.Structure):
+    _fields_ = [("iters", C.c_int), ("reliable_updates", C.c_int), ("converged", C.c_int), ("breakdown", C.c_int),
+                ("inner_applies", C.c_long), ("outer_applies", C.c_long), ("true_res", C.c_double),
+                ("seconds", C.c_double)]
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libmspcg.so and declare the prototypes.  Raises if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2104_05615_b200.build` (no CPU fallback exists)")
+    L = C.CDLL(LIB_PATH)
+    vp, dp, i, d = C.c_void_p, C.POINTER(C.c_double), C.c_int, C.c_double
+    L.mspcg_create.argtypes = [C.POINTER(vp), i, i, i, i, i, d, d, d, d, i, i, i, i]
+    L.mspcg_destroy.argtypes = [vp]
+    L.mspcg_last_error.argtypes = [vp]
+    L.mspcg_last_error.restype = C.c_char_p
+    L.mspcg_geometry.argtypes = [vp, C.POINTER(C.c_long)]
+    L.mspcg_get_matrix.argtypes = [vp, i, dp]
+    L.mspcg_workspace_bytes.argtypes = [vp, i, i, i, C.POINTER(C.c_size_t)]
+    L.mspcg_set_workspace.argtypes = [vp, vp, C.c_size_t, vp]
+    L.mspcg_load_gauge.argtypes = [vp, vp, i, vp]
+    L.mspcg_vec_bytes.argtypes = [vp, i]
+    L.mspcg_vec_bytes.restype = C.c_size_t
+    L.mspcg_pack.argtypes = [vp, vp, vp, i, vp]
+    L.mspcg_unpack.argtypes = [vp, vp, vp, i, vp]
+    L.mspcg_apply_MdagM.argtypes = [vp, vp, vp, i, i, vp]
+    L.mspcg_apply_precond.argtypes = [vp, vp, vp, i, i, i, i, vp]
+    L.mspcg_apply_MdagM_host.argtypes = [vp, vp, vp, i]
+    L.mspcg_apply_precond_host.argtypes = [vp, vp, vp, i, i, i]
+    L.mspcg_apply_A_block.argtypes = [vp, vp, vp, i, i, vp]
+    L.mspcg_set_reduced_ls.argtypes = [vp, i, dp, d]
+    L.mspcg_solve.argtypes = [vp, vp, vp, C.POINTER(SolveParams), C.POINTER(SolveStats), vp]
+    L.mspcg_launch_count.argtypes = [vp]
+    L.mspcg_launch_count.restype = C.c_long
+    _lib = L
+    return L
+
+
+class MspcgError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"mspcg error {code}: {msg}")
+        self.code = code
+
+
+_TORCH_DTYPE = None
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("no CUDA device: libmspcg has no CPU path")
+    return torch
+
+
+def _dtype(prec):
+    torch = _torch()
+    return {F64: torch.float64, F32: torch.float32, F16: torch.float16}[prec]
+
+
+class Mspcg:
+    """One mspcg_ctx.  Tensors passed in and out are torch CUDA tensors; the workspace is a torch uint8 tensor."""
+
+    def __init__(self, dims, Ls, b, c, M5, mf, block=None):
+        self.lib = load_library()
+        self.dims = tuple(int(x) for x in dims)
+        self.Ls = int(Ls)
+        self.block = tuple(int(x) for x in (block if block is not None else dims))
+        h = C.c_void_p()
+        rc = self.lib.mspcg_create(C.byref(h), *self.dims, self.Ls, b, c, M5, mf, *self.block)
+        if rc != OK:
+            raise MspcgError(rc, "mspcg_create rejected the parameters")
+        self.h = h
+        self.vh = int(np.prod(self.dims)) // 2
+        self.nreal = self.Ls * self.vh * 24
+        self.workspace = None
+        self.outer_prec = self.inner_prec = None
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.mspcg_destroy(self.h)
+            self.h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc, allow=()):
+        if rc != OK and rc not in allow:
+            raise MspcgError(rc, self.lib.mspcg_last_error(self.h).decode())
+        return rc
+
+    # ---- host-only queries -------------------------------------------------------------------------------------
+    def geometry(self):
+        out = (C.c_long * 5)()
+        self._check(self.lib.mspcg_geometry(self.h, out))
+        return dict(nblk=out[0], nE0=out[1], nE2=out[2], nO1=out[3], vh=out[4])
+
+    def matrix(self, which):
+        out = np.empty((self.Ls, self.Ls))
+        self._check(self.lib.mspcg_get_matrix(self.h, {"m5": 0, "mphi": 1, "m5inv": 2}[which],
+                                              out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out
+
+    def workspace_bytes(self, outer_prec=F32, inner_prec=F16, recon=18):
+        n = C.c_size_t()
+        self._check(self.lib.mspcg_workspace_bytes(self.h, outer_prec, inner_prec, recon, C.byref(n)))
+        self.outer_prec, self.inner_prec = outer_prec, inner_prec
+        return n.value
+
+    # ---- device set-up -----------------------------------------------------------------------------------------
+    def _stream(self):
+        return C.c_void_p(_torch().cuda.current_stream().cuda_stream)
+
+    def configure(self, outer_prec=F32, inner_prec=F16, recon=18):
+        torch = _torch()
+        n = self.workspace_bytes(outer_prec, inner_prec, recon)
+        self.workspace = torch.empty(n + 256, dtype=torch.uint8, device="cuda")
+        ptr = (self.workspace.data_ptr() + 255) & ~255
+        self._check(self.lib.mspcg_set_workspace(self.h, C.c_void_p(ptr), n, self._stream()))
+        return n
+
+    def load_gauge(self, U_abi, t_boundary=-1):
+        torch = _torch()
+        U = torch.as_tensor(np.ascontiguousarray(U_abi, dtype=np.float64)).cuda() if not hasattr(U_abi, "data_ptr") else U_abi
+        assert U.numel() == 4 * 2 * self.vh * 18 and U.dtype == torch.float64 and U.is_contiguous()
+        self._check(self.lib.mspcg_load_gauge(self.h, C.c_void_p(U.data_ptr()), int(t_boundary), self._stream()))
+        torch.cuda.current_stream().synchronize()  # U may be a temporary
+
+    # ---- vectors -----------------------------------------------------------------------------------------------
+    def new_native(self, prec):
+        torch = _torch()
+        return torch.empty(self.nreal, dtype=_dtype(prec), device="cuda")
+
+    def pack(self, abi, prec, out=None):
+        torch = _torch()
+        assert abi.dtype == torch.float64 and abi.numel() == self.nreal and abi.is_contiguous()
+        out = self.new_native(prec) if out is None else out
+        self._check(self.lib.mspcg_pack(self.h, C.c_void_p(abi.data_ptr()), C.c_void_p(out.data_ptr()), prec, self._stream()))
+        return out
+
+    def unpack(self, nat, prec, out=None):
+        torch = _torch()
+        out = torch.empty(self.nreal, dtype=torch.float64, device="cuda") if out is None else out
+        self._check(self.lib.mspcg_unpack(self.h, C.c_void_p(nat.data_ptr()), C.c_void_p(out.data_ptr()), prec, self._stream()))
+        return out
+
+    # ---- the hot path ------------------------------------------------------------------------------------------
+    def apply_MdagM(self, v, prec=F64, layout=LAYOUT_ABI, out=None):
+        torch = _torch()
+        out = torch.empty_like(v) if out is None else out
+        self._check(self.lib.mspcg_apply_MdagM(self.h, C.c_void_p(v.data_ptr()), C.c_void_p(out.data_ptr()), prec, layout, self._stream()))
+        return out
+
+    def apply_precond(self, r, n_inner, io_prec=F64, layout=LAYOUT_ABI, out=None, use_reduced=0):
+        torch = _torch()
+        out = torch.empty_like(r) if out is None else out
+        self._check(self.lib.mspcg_apply_precond(self.h, C.c_void_p(r.data_ptr()), C.c_void_p(out.data_ptr()), io_prec, layout,
+                                                 int(n_inner), int(use_reduced), self._stream()))
+        return out
+
+    def apply_A_block(self, v_abi, block, prec=None):
+        torch = _torch()
+        out = torch.empty_like(v_abi)
+        self._check(self.lib.mspcg_apply_A_block(self.h, C.c_void_p(v_abi.data_ptr()), C.c_void_p(out.data_ptr()), int(block),
+                                                 prec if prec is not None else self.inner_prec, self._stream()))
+        return out
+
+    def apply_MdagM_host(self, v_host, out_host, prec=F64):
+        self._check(self.lib.mspcg_apply_MdagM_host(self.h, C.c_void_p(v_host.data_ptr()), C.c_void_p(out_host.data_ptr()), prec))
+        return out_host
+
+    def apply_precond_host(self, r_host, z_host, n_inner, io_prec=F64, use_reduced=0):
+        self._check(self.lib.mspcg_apply_precond_host(self.h, C.c_void_p(r_host.data_ptr()), C.c_void_p(z_host.data_ptr()), io_prec,
+                                                      int(n_inner), int(use_reduced)))
+        return z_host
+
+    def solve(self, b_abi, x0_abi=None, tol=1e-10, max_iter=100000, use_precond=False, n_inner=6, sloppy_prec=F64,
+              delta=0.1, use_reduced_ls=False, history_len=0):
+        torch = _torch()
+        x = torch.zeros_like(b_abi) if x0_abi is None else x0_abi.clone()
+        hist = np.zeros(max(history_len, 1))
+        prm = SolveParams(tol, int(max_iter), int(use_precond), int(n_inner), int(sloppy_prec), delta, int(use_reduced_ls),
+                          int(history_len), hist.ctypes.data_as(C.POINTER(C.c_double)))
+        st = SolveStats()
+        rc = self.lib.mspcg_solve(self.h, C.c_void_p(b_abi.data_ptr()), C.c_void_p(x.data_ptr()), C.byref(prm), C.byref(st),
+                                  self._stream())
+        self._check(rc, allow=(ENOCONV, EBREAKDOWN))
+        stats = {k: getattr(st, k) for k, _ in SolveStats._fields_}
+        stats["rc"] = rc
+        stats["history"] = hist[:min(history_len, st.iters)].copy()
+        return x, stats
+
+    def launch_count(self):
+        return int(self.lib.mspcg_launch_count(self.h))

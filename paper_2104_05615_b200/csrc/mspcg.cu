@@ -1,0 +1,721 @@
+// mspcg.cu -- C ABI of libmspcg (include/mspcg.h): context, workspace carving, kernel launch sequences for
+// D^dag D (eq. 15-16), the multi-splitting preconditioner and the
+// outer PCG with reliable updates (Algorithm 1, 283-289).  All arithmetic runs in the kernels of
+// kernels.cuh; this file only sequences launches and moves scalars.  There is no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <type_traits>
+#include <string>
+#include <vector>
+
+#include "../../include/mspcg.h"
+#include "geometry.hpp"
+#include "kernels.cuh"
+
+using namespace mspcg;
+
+namespace {
+
+constexpr int KMAX = 32;  // most inner iterations per preconditioner application
+
+struct Arena {
+  char* base = nullptr; size_t off = 0; size_t cap = 0;
+  template <typename T> T* take(size_t n) {
+    off = (off + 255) & ~(size_t)255;
+    T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+    off += n * sizeof(T);
+    return p;
+  }
+  void* take_bytes(size_t n) { return take<char>(n); }
+};
+
+struct GeomDev { int *nbrE = nullptr, *nbrO = nullptr; short *cE = nullptr, *cO = nullptr, *origin = nullptr; };
+
+// One set of fifth-dimension matrices (device, transposed per chirality: m[ch][s'][s]) in one compute type.
+template <typename C> struct MatSet { C *K2 = nullptr, *K3a = nullptr, *K3b = nullptr, *K4 = nullptr, *K5 = nullptr; };
+struct HostMats { std::vector<double> K2, K3a, K3b, K4, K5; Mat A, F, Ainv; double diag, off; };
+
+// Everything one precision needs to apply D^dag D on one geometry.
+struct OpBuf {
+  int prec = 0, ng = 18;
+  void *linksE = nullptr, *linksO = nullptr; uint8_t *flipE = nullptr, *flipO = nullptr;
+  void *t1 = nullptr, *tO = nullptr, *y = nullptr, *w = nullptr;  // [nblk*nE0], [nblk*nO], [nblk*nE0], [nblk*nE]
+  bool have = false;
+};
+
+}  // namespace
+
+struct mspcg_ctx {
+  Lattice lat;
+  int Ls = 0, Ls_hat = 0;
+  double b = 0, c = 0, M5 = 0, mf = 0, alpha = 0, beta = 0, mu_shift = 0;
+  HostMats hm, hm_hat;
+  std::vector<double> T_host;
+  std::string err;
+  long launches = 0;
+  // configuration
+  int outer_prec = 0, inner_prec = 0, recon = 18;
+  bool configured = false, have_ws = false, have_gauge = false;
+  size_t ws_bytes = 0;
+  // device
+  GeomDev gfull, gblk;
+  int* e_int_to_cb = nullptr;
+  MatSet<double> md, md_hat; MatSet<float> mf32, mf32_hat;
+  OpBuf full64, fullS, blkI;     // full lattice fp64 / sloppy; block geometry in the inner precision
+  void *in_r = nullptr, *in_p = nullptr, *in_q = nullptr, *in_x = nullptr;   // inner CG vectors [V5h]
+  double *rho = nullptr, *pq = nullptr; float* scale = nullptr; double* sc = nullptr;  // device scalars
+  double* sc_host = nullptr;     // pinned
+  double *v_b = nullptr, *v_xhi = nullptr, *v_rhi = nullptr, *v_t64 = nullptr;   // solver, fp64 native
+  void *v_xlo = nullptr, *v_rlo = nullptr, *v_p = nullptr, *v_Ap = nullptr, *v_z = nullptr;  // solver, sloppy
+  void *stage_in = nullptr, *stage_out = nullptr;   // native staging for ABI-layout calls (fp64-sized)
+  double *abi_in = nullptr, *abi_out = nullptr;     // device ABI buffers for the *_host calls
+};
+
+namespace {
+
+int fail(mspcg_ctx* ctx, int code, const char* fmt, ...) {
+  if (ctx) {
+    char buf[512]; va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof(buf), fmt, ap); va_end(ap);
+    ctx->err = buf;
+  }
+  return code;
+}
+#define CUDA_OK(ctx, expr)                                                                              \
+  do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return fail(ctx, MSPCG_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_)); } while (0)
+
+bool ls_supported(int Ls) { return Ls == 4 || Ls == 6 || Ls == 8 || Ls == 12 || Ls == 16; }
+bool prec_ok(int p) { return p == MSPCG_F64 || p == MSPCG_F32 || p == MSPCG_F16; }
+long v5h(const mspcg_ctx* c, int Ls) { return c->lat.V4 / 2 * Ls; }
+size_t vec_bytes(const mspcg_ctx* c, int prec, int Ls) { return (size_t)v5h(c, Ls) * 24 * prec; }
+
+void transposed(const Mat& up, const Mat& lo, std::vector<double>& out) {
+  int n = up.n; out.resize((size_t)2 * n * n);
+  for (int s = 0; s < n; s++) for (int r = 0; r < n; r++) { out[(size_t)r * n + s] = up.at(s, r); out[(size_t)(n + r) * n + s] = lo.at(s, r); }
+}
+bool build_host_mats(HostMats& h, int Ls, double b, double c, double M5, double mf) {
+  double alpha = b * (4.0 - M5) + 1.0, beta = c * (4.0 - M5) - 1.0;
+  h.A = mat_bidiag(Ls, alpha, beta, mf);            // M5 on P+ (R3)
+  h.F = mat_bidiag(Ls, -0.5 * b, -0.5 * c, mf);     // Mphi on P+ (R1, R3)
+  if (!mat_inv(h.A, h.Ainv)) return false;
+  h.diag = -0.5 * b; h.off = -0.5 * c;
+  Mat At = mat_T(h.Ainv), Ft = mat_T(h.F);
+  transposed(mat_mul(h.F, h.Ainv), mat_mul(Ft, At), h.K2);     // Mphi M5^-1           (kernel 2 of eq. 16)
+  transposed(h.Ainv, At, h.K3a);                               // M5^-1                (kernel 3, first factor)
+  transposed(At, h.Ainv, h.K3b);                               // M5^-dag              (kernel 3, second factor)
+  transposed(mat_mul(At, Ft), mat_mul(h.Ainv, h.F), h.K4);     // M5^-dag Mphi^dag     (kernel 4)
+  transposed(Ft, h.F, h.K5);                                   // Mphi^dag             (kernel 5)
+  return true;
+}
+
+// ------------------------------------------------------------------------------------------------ workspace carving
+void carve_geom(Arena& a, GeomDev& g, const Geometry& h) {
+  g.nbrE = a.take<int>(h.nbrE.size()); g.nbrO = a.take<int>(h.nbrO.size());
+  g.cE = a.take<short>(h.cE.size()); g.cO = a.take<short>(h.cO.size()); g.origin = a.take<short>(h.origin.size());
+}
+template <typename C> void carve_mats(Arena& a, MatSet<C>& m, int Ls) {
+  size_t n = (size_t)2 * Ls * Ls;
+  m.K2 = a.take<C>(n); m.K3a = a.take<C>(n); m.K3b = a.take<C>(n); m.K4 = a.take<C>(n); m.K5 = a.take<C>(n);
+}
+void carve_op(Arena& a, OpBuf& o, const Geometry& g, int prec, int ng, int Ls) {
+  o.prec = prec; o.ng = ng; o.have = true;
+  size_t nblk = g.nblk;
+  o.linksE = a.take_bytes(nblk * g.nE * 8 * ng * prec); o.linksO = a.take_bytes(nblk * g.nO * 8 * ng * prec);
+  o.flipE = a.take<uint8_t>(nblk * g.nE); o.flipO = a.take<uint8_t>(nblk * g.nO);
+  size_t site = (size_t)Ls * 24 * prec;
+  o.t1 = a.take_bytes(nblk * g.nE0 * site); o.tO = a.take_bytes(nblk * g.nO * site);
+  o.y = a.take_bytes(nblk * g.nE0 * site); o.w = a.take_bytes(nblk * g.nE * site);
+}
+void carve(mspcg_ctx* c, Arena& a) {
+  const Lattice& L = c->lat;
+  carve_geom(a, c->gfull, L.full); carve_geom(a, c->gblk, L.blk);
+  c->e_int_to_cb = a.take<int>(L.e_int_to_cb.size());
+  carve_mats(a, c->md, c->Ls); carve_mats(a, c->mf32, c->Ls);
+  if (c->Ls_hat) { carve_mats(a, c->md_hat, c->Ls_hat); carve_mats(a, c->mf32_hat, c->Ls_hat); }
+  c->rho = a.take<double>((size_t)(KMAX + 1) * L.nblk); c->pq = a.take<double>((size_t)KMAX * L.nblk);
+  c->scale = a.take<float>(L.nblk); c->sc = a.take<double>(16);
+  carve_op(a, c->full64, L.full, MSPCG_F64, 18, c->Ls);
+  if (c->outer_prec != MSPCG_F64) carve_op(a, c->fullS, L.full, c->outer_prec, c->recon, c->Ls);
+  carve_op(a, c->blkI, L.blk, c->inner_prec, c->inner_prec == MSPCG_F64 ? 18 : c->recon, c->Ls);
+  size_t ni = vec_bytes(c, c->inner_prec, c->Ls);
+  c->in_r = a.take_bytes(ni); c->in_p = a.take_bytes(ni); c->in_q = a.take_bytes(ni);
+  c->in_x = a.take_bytes(vec_bytes(c, c->inner_prec == MSPCG_F64 ? MSPCG_F64 : MSPCG_F32, c->Ls));
+  size_t n64 = vec_bytes(c, MSPCG_F64, c->Ls), nS = vec_bytes(c, c->outer_prec, c->Ls);
+  c->v_b = (double*)a.take_bytes(n64); c->v_xhi = (double*)a.take_bytes(n64); c->v_rhi = (double*)a.take_bytes(n64);
+  c->v_t64 = (double*)a.take_bytes(n64);
+  c->v_xlo = a.take_bytes(nS); c->v_rlo = a.take_bytes(nS); c->v_p = a.take_bytes(nS); c->v_Ap = a.take_bytes(nS);
+  c->v_z = a.take_bytes(nS);
+  c->stage_in = a.take_bytes(n64); c->stage_out = a.take_bytes(n64);
+  c->abi_in = (double*)a.take_bytes(n64); c->abi_out = (double*)a.take_bytes(n64);
+}
+
+// ------------------------------------------------------------------------------------------------ kernel launchers
+#define DISPATCH_LS(LSV, ...)                                            \
+  switch (LSV) {                                                         \
+    case 4: { constexpr int LS = 4; __VA_ARGS__; } break;                \
+    case 6: { constexpr int LS = 6; __VA_ARGS__; } break;                \
+    case 8: { constexpr int LS = 8; __VA_ARGS__; } break;                \
+    case 12: { constexpr int LS = 12; __VA_ARGS__; } break;              \
+    default: { constexpr int LS = 16; __VA_ARGS__; } break;              \
+  }
+
+template <typename T, int LS, int EPI> size_t hop_smem() {
+  typedef typename ST<T>::C C; typedef Smem<C, LS> SM;
+  return sizeof(C) * ((size_t)SM::NS * SM::USTRIDE + (size_t)SM::NS * SM::SSTRIDE + (size_t)(EPI == EPI_K3 ? 4 : 2) * LS * LS) + sizeof(int) * SM::NS * 8;
+}
+template <typename T, int LS, int EPI>
+cudaError_t launch_hop(mspcg_ctx* c, const HopArgs<T>& a, int nblk, cudaStream_t st) {
+  static bool attr = false;
+  const size_t sm = hop_smem<T, LS, EPI>();
+  if (!attr) { cudaFuncSetAttribute(k_hop<T, LS, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); attr = true; }
+  dim3 block(LS, Tile<LS>::NS), grid((a.n_out + Tile<LS>::NS - 1) / Tile<LS>::NS, nblk);
+  k_hop<T, LS, EPI><<<grid, block, sm, st>>>(a);
+  c->launches++;
+  return cudaPeekAtLastError();
+}
+template <typename T, int LS>
+cudaError_t launch_mphi(mspcg_ctx* c, const MphiArgs<T>& a, int nblk, cudaStream_t st) {
+  typedef typename ST<T>::C C; typedef Smem<C, LS> SM;
+  static bool attr = false;
+  const size_t sm = sizeof(C) * (size_t)SM::NS * SM::SSTRIDE;
+  if (!attr) { cudaFuncSetAttribute(k_mphi<T, LS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); attr = true; }
+  dim3 block(LS, Tile<LS>::NS), grid((unsigned)((a.n_sites + Tile<LS>::NS - 1) / Tile<LS>::NS), nblk);
+  k_mphi<T, LS><<<grid, block, sm, st>>>(a);
+  c->launches++;
+  return cudaPeekAtLastError();
+}
+
+template <typename C> struct MatPick;
+template <> struct MatPick<double> { static const MatSet<double>& get(const mspcg_ctx* c, bool hat) { return hat ? c->md_hat : c->md; } };
+template <> struct MatPick<float> { static const MatSet<float>& get(const mspcg_ctx* c, bool hat) { return hat ? c->mf32_hat : c->mf32; } };
+
+// Geometry view handed to the operator sequence: tables + per-precision buffers, possibly offset to one block.
+template <typename T> struct OpView {
+  int nblk, nE0, nE, nO, ng, Ls; bool hat;
+  const int *nbrE, *nbrO;
+  const T *linksE, *linksO; const uint8_t *flipE, *flipO;
+  T *t1, *tO, *y, *w;
+};
+template <typename T> OpView<T> make_view(const mspcg_ctx* c, const OpBuf& o, const Geometry& g, const GeomDev& gd, int Ls, bool hat) {
+  OpView<T> v;
+  v.nblk = g.nblk; v.nE0 = g.nE0; v.nE = g.nE; v.nO = g.nO; v.ng = o.ng; v.Ls = Ls; v.hat = hat;
+  v.nbrE = gd.nbrE; v.nbrO = gd.nbrO;
+  v.linksE = (const T*)o.linksE; v.linksO = (const T*)o.linksO; v.flipE = o.flipE; v.flipO = o.flipO;
+  v.t1 = (T*)o.t1; v.tO = (T*)o.tO; v.y = (T*)o.y; v.w = (T*)o.w;
+  return v;
+}
+template <typename T> OpView<T> one_block(const OpView<T>& v, int blk) {
+  OpView<T> o = v; o.nblk = 1;
+  o.linksE = v.linksE + (size_t)blk * v.nE * 8 * v.ng; o.linksO = v.linksO + (size_t)blk * v.nO * 8 * v.ng;
+  o.flipE = v.flipE + (size_t)blk * v.nE; o.flipO = v.flipO + (size_t)blk * v.nO;
+  return o;
+}
+
+// q = D^dag D p on the view's geometry.  `mp` describes kernel 1 (Mphi, possibly fused with a p-update; its `t`,
+// `n_sites`, matrix entries are filled here).  If dot_out != null: dot_out[blk] += Re<p, q>.
+//   K1  t1 = Mphi p                              K2  tO = (Mphi M5^-1) D^w t1
+//   K3  y = p - M5^-1 D^w tO ; w = M5^-dag y     K4  tO = (M5^-dag Mphi^dag) D^w^dag w
+//   K5  q = y - Mphi^dag D^w^dag tO              (eq. 16; on a Dirichlet block the stage outputs live on
+//                                                 the site sets d<=1, d<=2, d<=1, d=0 of PAPER.md:226)
+template <typename T, int LS>
+cudaError_t apply_normal(mspcg_ctx* c, const OpView<T>& v, MphiArgs<T> mp, const T* p, T* q, double* dot_out, cudaStream_t st) {
+  typedef typename ST<T>::C C;
+  const MatSet<C>& m = MatPick<C>::get(c, v.hat);
+  const HostMats& hm = v.hat ? c->hm_hat : c->hm;
+  cudaError_t e;
+  mp.t = v.t1; mp.n_sites = v.nE0; mp.diag = (C)hm.diag; mp.off = (C)hm.off; mp.mf = (C)c->mf;
+  if ((e = launch_mphi<T, LS>(c, mp, v.nblk, st)) != cudaSuccess) return e;
+  HopArgs<T> a;
+  memset(&a, 0, sizeof(a));
+  a.ng = v.ng;
+  // K2
+  a.in = v.t1; a.in_stride = v.nE0; a.n_in_limit = v.nE0; a.out = v.tO; a.out_stride = v.nO; a.n_out = v.nO;
+  a.nbr = v.nbrO; a.links = v.linksO; a.flip = v.flipO; a.link_stride = v.nO; a.mat1 = m.K2; a.sg = (C)1;
+  if ((e = launch_hop<T, LS, EPI_PLAIN>(c, a, v.nblk, st)) != cudaSuccess) return e;
+  // K3
+  a.in = v.tO; a.in_stride = v.nO; a.n_in_limit = v.nO; a.out = v.w; a.out_stride = v.nE; a.n_out = v.nE;
+  a.out2 = v.y; a.out2_stride = v.nE0; a.n_out2 = v.nE0; a.aux = p; a.aux_stride = v.nE0; a.n_aux = v.nE0;
+  a.nbr = v.nbrE; a.links = v.linksE; a.flip = v.flipE; a.link_stride = v.nE; a.mat1 = m.K3a; a.mat2 = m.K3b;
+  if ((e = launch_hop<T, LS, EPI_K3>(c, a, v.nblk, st)) != cudaSuccess) return e;
+  // K4
+  a.in = v.w; a.in_stride = v.nE; a.n_in_limit = v.nE; a.out = v.tO; a.out_stride = v.nO; a.n_out = v.nO;
+  a.out2 = nullptr; a.aux = nullptr; a.n_aux = 0; a.nbr = v.nbrO; a.links = v.linksO; a.flip = v.flipO; a.link_stride = v.nO;
+  a.mat1 = m.K4; a.mat2 = nullptr; a.sg = (C)-1;
+  if ((e = launch_hop<T, LS, EPI_PLAIN>(c, a, v.nblk, st)) != cudaSuccess) return e;
+  // K5
+  a.in = v.tO; a.in_stride = v.nO; a.n_in_limit = v.nO; a.out = q; a.out_stride = v.nE0; a.n_out = v.nE0;
+  a.aux = v.y; a.aux_stride = v.nE0; a.n_aux = v.nE0; a.dotv = p; a.dotv_stride = v.nE0; a.dot_out = dot_out; a.dot_stride = 1;
+  a.nbr = v.nbrE; a.links = v.linksE; a.flip = v.flipE; a.link_stride = v.nE; a.mat1 = m.K5;
+  return launch_hop<T, LS, EPI_XPAY>(c, a, v.nblk, st);
+}
+
+template <typename T> MphiArgs<T> mphi_plain(const T* in) { MphiArgs<T> a; memset(&a, 0, sizeof(a)); a.in = in; a.mode = 0; return a; }
+
+inline dim3 grid_sites(long n_sites, int Ls, int nblk, int threads = 128) { return dim3((unsigned)((n_sites * Ls + threads - 1) / threads), nblk); }
+
+template <typename TA, typename TB>
+cudaError_t convert(mspcg_ctx* c, const void* a, void* b, long n_sites, int Ls, int nblk, const float* scale, int invert, double factor, cudaStream_t st) {
+  k_convert<TA, TB><<<grid_sites(n_sites, Ls, nblk), 128, 0, st>>>((const TA*)a, (TB*)b, n_sites, Ls, scale, invert, factor);
+  c->launches++;
+  return cudaPeekAtLastError();
+}
+cudaError_t convert_any(mspcg_ctx* c, const void* a, int pa, void* b, int pb, long n_sites, int Ls, cudaStream_t st) {
+#define CV(PA, TA, PB, TB) if (pa == PA && pb == PB) return convert<TA, TB>(c, a, b, n_sites, Ls, 1, nullptr, 0, 1.0, st);
+  CV(8, double, 8, double) CV(8, double, 4, float) CV(8, double, 2, __half)
+  CV(4, float, 8, double) CV(4, float, 4, float) CV(4, float, 2, __half)
+  CV(2, __half, 8, double) CV(2, __half, 4, float) CV(2, __half, 2, __half)
+#undef CV
+  return cudaErrorInvalidValue;
+}
+
+// ---------------------------------------------------------------------------------------- the preconditioner (A7, A8)
+template <typename TIO, typename T, int LS>
+cudaError_t precond_impl(mspcg_ctx* c, const TIO* r_in, TIO* z_out, int k, cudaStream_t st) {
+  typedef typename std::conditional<sizeof(T) == 8, double, float>::type TX;
+  const Geometry& g = c->lat.blk;
+  const int nblk = g.nblk;
+  OpView<T> v = make_view<T>(c, c->blkI, g, c->gblk, LS, false);
+  cudaError_t e;
+  if ((e = cudaMemsetAsync(c->rho, 0, sizeof(double) * (size_t)(KMAX + 1) * nblk, st)) != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(c->pq, 0, sizeof(double) * (size_t)KMAX * nblk, st)) != cudaSuccess) return e;
+  const float* scale = nullptr;
+  if (sizeof(T) == 2) {   // fp16 storage: rescale every block's right-hand side to max-abs 1 (R14)
+    if ((e = cudaMemsetAsync(c->scale, 0, sizeof(float) * nblk, st)) != cudaSuccess) return e;
+    k_maxabs<TIO><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(r_in, g.nE0, LS, c->scale);
+    c->launches++;
+    scale = c->scale;
+  }
+  T *r = (T*)c->in_r, *p = (T*)c->in_p, *q = (T*)c->in_q; TX* x = (TX*)c->in_x;
+  k_pre_begin<TIO, T><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(r_in, r, g.nE0, LS, scale, c->rho);
+  c->launches++;
+  for (int it = 0; it < k; it++) {
+    MphiArgs<T> mp; memset(&mp, 0, sizeof(mp));
+    mp.in = r; mp.p = p; mp.mode = 2; mp.it = it; mp.nblk = nblk; mp.rho = c->rho; mp.pq = c->pq;
+    if ((e = apply_normal<T, LS>(c, v, mp, p, q, c->pq + (size_t)it * nblk, st)) != cudaSuccess) return e;
+    k_inner_update<T, TX, TIO><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(p, q, r, x, z_out, g.nE0, LS, it, nblk, it == k - 1,
+                                                                          c->rho, c->pq, scale);
+    c->launches++;
+  }
+  return cudaPeekAtLastError();
+}
+
+template <typename TIO>
+cudaError_t precond_dispatch(mspcg_ctx* c, const TIO* r, TIO* z, int k, cudaStream_t st) {
+  const int Ls = c->Ls;
+  switch (c->inner_prec) {
+    case MSPCG_F64: DISPATCH_LS(Ls, return (precond_impl<TIO, double, LS>(c, r, z, k, st)));
+    case MSPCG_F32: DISPATCH_LS(Ls, return (precond_impl<TIO, float, LS>(c, r, z, k, st)));
+    default: DISPATCH_LS(Ls, return (precond_impl<TIO, __half, LS>(c, r, z, k, st)));
+  }
+  return cudaErrorInvalidValue;
+}
+cudaError_t precond_any(mspcg_ctx* c, const void* r, void* z, int io_prec, int k, cudaStream_t st) {
+  if (io_prec == MSPCG_F64) return precond_dispatch<double>(c, (const double*)r, (double*)z, k, st);
+  if (io_prec == MSPCG_F32) return precond_dispatch<float>(c, (const float*)r, (float*)z, k, st);
+  return precond_dispatch<__half>(c, (const __half*)r, (__half*)z, k, st);
+}
+
+// ------------------------------------------------------------------------------------------- full-lattice D^dag D
+template <typename T>
+cudaError_t normal_full(mspcg_ctx* c, const OpBuf& ob, const T* p, T* q, MphiArgs<T> mp, double* dot_out, cudaStream_t st) {
+  OpView<T> v = make_view<T>(c, ob, c->lat.full, c->gfull, c->Ls, false);
+  DISPATCH_LS(c->Ls, return (apply_normal<T, LS>(c, v, mp, p, q, dot_out, st)));
+  return cudaErrorInvalidValue;
+}
+const OpBuf* full_buf(const mspcg_ctx* c, int prec) {
+  if (prec == MSPCG_F64) return &c->full64;
+  if (prec == c->outer_prec && c->fullS.have) return &c->fullS;
+  return nullptr;
+}
+cudaError_t normal_full_any(mspcg_ctx* c, int prec, const void* p, void* q, double* dot_out, cudaStream_t st) {
+  const OpBuf* ob = full_buf(c, prec);
+  if (!ob) return cudaErrorInvalidValue;
+  if (prec == MSPCG_F64) return normal_full<double>(c, *ob, (const double*)p, (double*)q, mphi_plain<double>((const double*)p), dot_out, st);
+  if (prec == MSPCG_F32) return normal_full<float>(c, *ob, (const float*)p, (float*)q, mphi_plain<float>((const float*)p), dot_out, st);
+  return normal_full<__half>(c, *ob, (const __half*)p, (__half*)q, mphi_plain<__half>((const __half*)p), dot_out, st);
+}
+
+cudaError_t pack_any(mspcg_ctx* c, const double* abi, void* nat, int prec, int to_native, cudaStream_t st) {
+  const long Vh = c->lat.V4 / 2;
+#define PK(TT) DISPATCH_LS(c->Ls, { dim3 block(LS, Tile<LS>::NS), grid((unsigned)((Vh + Tile<LS>::NS - 1) / Tile<LS>::NS)); \
+    k_pack<TT, LS><<<grid, block, 0, st>>>(abi, (TT*)nat, c->e_int_to_cb, Vh, to_native); })
+  if (prec == MSPCG_F64) PK(double) else if (prec == MSPCG_F32) PK(float) else PK(__half)
+#undef PK
+  c->launches++;
+  return cudaPeekAtLastError();
+}
+
+template <typename T>
+cudaError_t build_links(mspcg_ctx* c, const double* U, OpBuf& o, const Geometry& g, const GeomDev& gd, int tb, cudaStream_t st) {
+  const Lattice& L = c->lat;
+  long nE = (long)g.nblk * g.nE, nO = (long)g.nblk * g.nO;
+  k_build_links<T><<<(unsigned)((nE + 127) / 128), 128, 0, st>>>(U, (T*)o.linksE, o.flipE, gd.cE, gd.origin, g.nE, g.nblk, L.L[0], L.L[1], L.L[2], L.L[3], tb, o.ng);
+  k_build_links<T><<<(unsigned)((nO + 127) / 128), 128, 0, st>>>(U, (T*)o.linksO, o.flipO, gd.cO, gd.origin, g.nO, g.nblk, L.L[0], L.L[1], L.L[2], L.L[3], tb, o.ng);
+  c->launches += 2;
+  return cudaPeekAtLastError();
+}
+cudaError_t build_links_any(mspcg_ctx* c, const double* U, OpBuf& o, const Geometry& g, const GeomDev& gd, int tb, cudaStream_t st) {
+  if (o.prec == MSPCG_F64) return build_links<double>(c, U, o, g, gd, tb, st);
+  if (o.prec == MSPCG_F32) return build_links<float>(c, U, o, g, gd, tb, st);
+  return build_links<__half>(c, U, o, g, gd, tb, st);
+}
+
+template <typename C> cudaError_t upload_mats(const MatSet<C>& m, const HostMats& h, cudaStream_t st) {
+  const std::vector<double>* src[5] = {&h.K2, &h.K3a, &h.K3b, &h.K4, &h.K5};
+  C* dst[5] = {m.K2, m.K3a, m.K3b, m.K4, m.K5};
+  for (int i = 0; i < 5; i++) {
+    std::vector<C> tmp(src[i]->begin(), src[i]->end());
+    cudaError_t e = cudaMemcpyAsync(dst[i], tmp.data(), tmp.size() * sizeof(C), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return e;
+    cudaStreamSynchronize(st);  // tmp goes out of scope
+  }
+  return cudaSuccess;
+}
+template <typename V> cudaError_t up(void* dst, const std::vector<V>& src, cudaStream_t st) {
+  return cudaMemcpyAsync(dst, src.data(), src.size() * sizeof(V), cudaMemcpyHostToDevice, st);
+}
+
+int check_ready(mspcg_ctx* c, bool need_gauge) {
+  if (!c) return MSPCG_EINVAL;
+  if (!c->have_ws) return fail(c, MSPCG_ENOWORKSPACE, "mspcg_set_workspace has not been called");
+  if (need_gauge && !c->have_gauge) return fail(c, MSPCG_ENOGAUGE, "mspcg_load_gauge has not been called");
+  return MSPCG_OK;
+}
+
+// scalar helpers for the outer loop: zero n device doubles / read them back synchronously
+cudaError_t sc_zero(mspcg_ctx* c, int n, cudaStream_t st) { return cudaMemsetAsync(c->sc, 0, sizeof(double) * n, st); }
+cudaError_t sc_read(mspcg_ctx* c, int n, cudaStream_t st) {
+  cudaError_t e = cudaMemcpyAsync(c->sc_host, c->sc, sizeof(double) * n, cudaMemcpyDeviceToHost, st);
+  if (e != cudaSuccess) return e;
+  return cudaStreamSynchronize(st);
+}
+template <typename T> cudaError_t dot2(mspcg_ctx* c, const T* a, const T* b, const T* cc, long nreal, cudaStream_t st) {
+  const long nchunk = nreal / ST<T>::PER;
+  long blocks = (nchunk + 255) / 256; if (blocks > 148 * 16) blocks = 148 * 16;
+  k_dot2<T><<<(unsigned)blocks, 256, 0, st>>>(a, b, cc, nchunk, c->sc);
+  c->launches++;
+  return cudaPeekAtLastError();
+}
+template <typename T> cudaError_t axpby(mspcg_ctx* c, double a, const T* x, double b, T* y, long nreal, cudaStream_t st) {
+  const long nchunk = nreal / ST<T>::PER;
+  k_axpby<T><<<(unsigned)((nchunk + 255) / 256), 256, 0, st>>>(a, x, b, y, nchunk);
+  c->launches++;
+  return cudaPeekAtLastError();
+}
+
+// ------------------------------------------------------------------------------------------------ outer PCG (A11)
+#define SOLVE_CUDA(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) return fail(c, MSPCG_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_)); } while (0)
+
+template <typename TS>
+int solve_impl(mspcg_ctx* c, const double* b_abi, double* x_abi, const mspcg_solve_params* prm, mspcg_solve_stats* stt, cudaStream_t st) {
+  const int Ls = c->Ls;
+  const long nreal = v5h(c, Ls) * 24;
+  const long Vh = c->lat.V4 / 2;
+  const bool sloppy = sizeof(TS) != 8;
+  const int sp = (int)sizeof(TS);
+  const OpBuf& obS = sloppy ? c->fullS : c->full64;
+  double *b = c->v_b, *xhi = c->v_xhi, *rhi = c->v_rhi, *t64 = c->v_t64;
+  TS *xlo = (TS*)c->v_xlo, *rlo = (TS*)c->v_rlo, *p = (TS*)c->v_p, *Ap = (TS*)c->v_Ap;
+  TS* z = prm->use_precond ? (TS*)c->v_z : rlo;
+  memset(stt, 0, sizeof(*stt));
+  const long launches0 = c->launches;
+  cudaEvent_t ev0, ev1;
+  SOLVE_CUDA(cudaEventCreate(&ev0)); SOLVE_CUDA(cudaEventCreate(&ev1));
+  SOLVE_CUDA(cudaEventRecord(ev0, st));
+  SOLVE_CUDA(pack_any(c, b_abi, b, MSPCG_F64, 1, st));
+  SOLVE_CUDA(pack_any(c, x_abi, xhi, MSPCG_F64, 1, st));
+  SOLVE_CUDA(sc_zero(c, 2, st));
+  SOLVE_CUDA(dot2<double>(c, b, b, nullptr, nreal, st));
+  SOLVE_CUDA(sc_read(c, 1, st));
+  const double bnorm = std::sqrt(c->sc_host[0]);
+  int k = 0, rc = MSPCG_OK;
+  auto true_residual = [&](double* rn) -> cudaError_t {   // rhi = b - A xhi in fp64; *rn = |rhi|
+    cudaError_t e;
+    if ((e = normal_full<double>(c, c->full64, xhi, t64, mphi_plain<double>(xhi), nullptr, st)) != cudaSuccess) return e;
+    stt->outer_applies++;
+    if ((e = cudaMemcpyAsync(rhi, b, sizeof(double) * nreal, cudaMemcpyDeviceToDevice, st)) != cudaSuccess) return e;
+    if ((e = axpby<double>(c, -1.0, t64, 1.0, rhi, nreal, st)) != cudaSuccess) return e;
+    if ((e = sc_zero(c, 1, st)) != cudaSuccess) return e;
+    if ((e = dot2<double>(c, rhi, rhi, nullptr, nreal, st)) != cudaSuccess) return e;
+    if ((e = sc_read(c, 1, st)) != cudaSuccess) return e;
+    *rn = std::sqrt(c->sc_host[0]);
+    return cudaSuccess;
+  };
+  if (bnorm == 0.0) {  // R15: b = 0 -> x = 0
+    SOLVE_CUDA(cudaMemsetAsync(x_abi, 0, sizeof(double) * nreal, st));
+    stt->converged = 1;
+  } else {
+    double rnorm = 0, maxr, rz = 0, alpha = 0, beta = 0;
+    SOLVE_CUDA(true_residual(&rnorm));                       // r0 = b - A x0 (R15)
+    SOLVE_CUDA(convert_any(c, rhi, 8, rlo, sp, Vh, Ls, st));
+    SOLVE_CUDA(cudaMemsetAsync(xlo, 0, sizeof(TS) * nreal, st));
+    maxr = rnorm;
+    if (rnorm <= prm->tol * bnorm) stt->converged = 1;
+    else {
+      if (prm->use_precond) { SOLVE_CUDA(precond_any(c, rlo, z, sp, prm->n_inner, st)); stt->inner_applies += (long)prm->n_inner * c->lat.nblk; }
+      SOLVE_CUDA(cudaMemcpyAsync(p, z, sizeof(TS) * nreal, cudaMemcpyDeviceToDevice, st));   // p0 = z0
+      SOLVE_CUDA(sc_zero(c, 2, st));
+      SOLVE_CUDA(dot2<TS>(c, rlo, z, nullptr, nreal, st));
+      SOLVE_CUDA(sc_read(c, 1, st));
+      rz = c->sc_host[0];
+    }
+    while (!stt->converged && k < prm->max_iter) {
+      // Ap = A p; for k > 0 the update p = z + beta p is fused into kernel 1
+      MphiArgs<TS> mp; memset(&mp, 0, sizeof(mp));
+      if (k == 0) { mp.in = p; mp.mode = 0; } else { mp.in = z; mp.p = p; mp.mode = 1; mp.beta = beta; }
+      SOLVE_CUDA(sc_zero(c, 4, st));
+      SOLVE_CUDA(normal_full<TS>(c, obS, p, Ap, mp, c->sc, st));
+      stt->outer_applies++;
+      SOLVE_CUDA(sc_read(c, 1, st));
+      const double pAp = c->sc_host[0];
+      if (!(pAp > 0.0)) { stt->breakdown = 1; rc = MSPCG_EBREAKDOWN; break; }
+      alpha = rz / pAp;                                       // alpha_k = <r_k,z_k>/<p_k,A p_k>
+      { const long nchunk = nreal / ST<TS>::PER;
+        k_outer_update<TS><<<(unsigned)((nchunk + 255) / 256), 256, 0, st>>>(p, Ap, rlo, xlo, nchunk, alpha, c->sc + 1);
+        c->launches++; }
+      SOLVE_CUDA(sc_read(c, 2, st));
+      rnorm = std::sqrt(c->sc_host[1]);
+      k++;
+      if (prm->history && k <= prm->history_len) prm->history[k - 1] = rnorm / bnorm;
+      if (!(rnorm == rnorm)) { stt->breakdown = 1; rc = MSPCG_EBREAKDOWN; break; }
+      bool replaced = false;
+      if (rnorm <= prm->tol * bnorm || (sloppy && rnorm < prm->delta * maxr)) {
+        // R17 residual replacement / R15 confirmation with the true residual
+        SOLVE_CUDA(convert_any(c, xlo, sp, t64, 8, Vh, Ls, st));
+        SOLVE_CUDA(axpby<double>(c, 1.0, t64, 1.0, xhi, nreal, st));
+        SOLVE_CUDA(cudaMemsetAsync(xlo, 0, sizeof(TS) * nreal, st));
+        SOLVE_CUDA(true_residual(&rnorm));
+        SOLVE_CUDA(convert_any(c, rhi, 8, rlo, sp, Vh, Ls, st));
+        maxr = rnorm; stt->reliable_updates++; replaced = true;
+        if (rnorm <= prm->tol * bnorm) { stt->converged = 1; break; }
+      }
+      if (rnorm > maxr) maxr = rnorm;
+      if (prm->use_precond) { SOLVE_CUDA(precond_any(c, rlo, z, sp, prm->n_inner, st)); stt->inner_applies += (long)prm->n_inner * c->lat.nblk; }
+      SOLVE_CUDA(sc_zero(c, 2, st));
+      SOLVE_CUDA(dot2<TS>(c, z, rlo, Ap, nreal, st));
+      SOLVE_CUDA(sc_read(c, 2, st));
+      const double rz_new = c->sc_host[0], zAp = c->sc_host[1];
+      beta = replaced ? rz_new / rz : (rz_new + alpha * zAp) / rz;   // eq. 18 in the form of R16
+      rz = rz_new;
+    }
+    if (!stt->converged && rc == MSPCG_OK) rc = MSPCG_ENOCONV;
+    // x = x_hi + x_lo, true residual, unpack
+    SOLVE_CUDA(convert_any(c, xlo, sp, t64, 8, Vh, Ls, st));
+    SOLVE_CUDA(axpby<double>(c, 1.0, t64, 1.0, xhi, nreal, st));
+    double rn = 0;
+    SOLVE_CUDA(true_residual(&rn));
+    stt->outer_applies--;   // the closing residual check is bookkeeping, not part of the iteration
+    stt->true_res = rn / bnorm;
+    SOLVE_CUDA(pack_any(c, x_abi, xhi, MSPCG_F64, 0, st));
+  }
+  stt->iters = k;
+  SOLVE_CUDA(cudaEventRecord(ev1, st));
+  SOLVE_CUDA(cudaEventSynchronize(ev1));
+  float ms = 0; cudaEventElapsedTime(&ms, ev0, ev1);
+  stt->seconds = ms * 1e-3;
+  cudaEventDestroy(ev0); cudaEventDestroy(ev1);
+  (void)launches0;
+  return rc == MSPCG_OK ? MSPCG_OK : fail(c, rc, rc == MSPCG_ENOCONV ? "max_iter reached" : "breakdown: <p,Ap> <= 0 or NaN");
+}
+
+}  // namespace
+
+// ================================================================================================== C ABI
+extern "C" {
+
+int mspcg_create(mspcg_ctx** out, int Lx, int Ly, int Lz, int Lt, int Ls, double b, double c, double M5, double mf,
+                 int Bx, int By, int Bz, int Bt) {
+  if (!out) return MSPCG_EINVAL;
+  *out = nullptr;
+  if (!ls_supported(Ls)) return MSPCG_EINVAL;
+  if (b * (4.0 - M5) + 1.0 == 0.0) return MSPCG_EINVAL;
+  mspcg_ctx* ctx = new (std::nothrow) mspcg_ctx();
+  if (!ctx) return MSPCG_ENOMEM;
+  const int L[4] = {Lx, Ly, Lz, Lt}, B[4] = {Bx, By, Bz, Bt};
+  if (!build_lattice(ctx->lat, L, B)) { delete ctx; return MSPCG_EINVAL; }
+  ctx->Ls = Ls; ctx->b = b; ctx->c = c; ctx->M5 = M5; ctx->mf = mf;
+  ctx->alpha = b * (4.0 - M5) + 1.0; ctx->beta = c * (4.0 - M5) - 1.0;
+  if (!build_host_mats(ctx->hm, Ls, b, c, M5, mf)) { delete ctx; return MSPCG_EINVAL; }
+  *out = ctx;
+  return MSPCG_OK;
+}
+
+int mspcg_destroy(mspcg_ctx* ctx) {
+  if (!ctx) return MSPCG_EINVAL;
+  if (ctx->sc_host) cudaFreeHost(ctx->sc_host);
+  delete ctx;
+  return MSPCG_OK;
+}
+
+const char* mspcg_last_error(const mspcg_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int mspcg_geometry(const mspcg_ctx* ctx, long out[5]) {
+  if (!ctx || !out) return MSPCG_EINVAL;
+  out[0] = ctx->lat.nblk; out[1] = ctx->lat.blk.nE0; out[2] = ctx->lat.blk.nE; out[3] = ctx->lat.blk.nO; out[4] = ctx->lat.V4 / 2;
+  return MSPCG_OK;
+}
+
+int mspcg_get_matrix(const mspcg_ctx* ctx, int which, double* out_host) {
+  if (!ctx || !out_host || which < 0 || which > 2) return MSPCG_EINVAL;
+  const Mat& m = which == 0 ? ctx->hm.A : which == 1 ? ctx->hm.F : ctx->hm.Ainv;
+  memcpy(out_host, m.a.data(), m.a.size() * sizeof(double));
+  return MSPCG_OK;
+}
+
+int mspcg_set_reduced_ls(mspcg_ctx* ctx, int Ls_hat, const double* T_host, double mu) {
+  if (!ctx) return MSPCG_EINVAL;
+  if (ctx->configured) return fail(ctx, MSPCG_EINVAL, "mspcg_set_reduced_ls must precede mspcg_workspace_bytes");
+  if (!ls_supported(Ls_hat) || Ls_hat > ctx->Ls || !T_host) return fail(ctx, MSPCG_EINVAL, "unsupported Ls_hat");
+  if (!build_host_mats(ctx->hm_hat, Ls_hat, ctx->b, ctx->c, ctx->M5, ctx->mf)) return fail(ctx, MSPCG_EINVAL, "singular M5 at Ls_hat");
+  ctx->Ls_hat = Ls_hat; ctx->mu_shift = mu;
+  ctx->T_host.assign(T_host, T_host + (size_t)4 * Ls_hat * 4 * ctx->Ls * 2);
+  return fail(ctx, MSPCG_EINVAL, "reduced-Ls apply is not built yet (SURVEY 8(a) A10)");
+}
+
+int mspcg_workspace_bytes(mspcg_ctx* ctx, int outer_prec, int inner_prec, int recon, size_t* bytes) {
+  if (!ctx || !bytes) return MSPCG_EINVAL;
+  if (!prec_ok(outer_prec) || !prec_ok(inner_prec) || (recon != 18 && recon != 12)) return fail(ctx, MSPCG_EINVAL, "bad precision or recon");
+  if (ctx->have_ws) return fail(ctx, MSPCG_EINVAL, "workspace already set");
+  ctx->outer_prec = outer_prec; ctx->inner_prec = inner_prec; ctx->recon = recon; ctx->configured = true;
+  Arena a;
+  carve(ctx, a);
+  ctx->ws_bytes = (a.off + 255) & ~(size_t)255;
+  *bytes = ctx->ws_bytes;
+  return MSPCG_OK;
+}
+
+int mspcg_set_workspace(mspcg_ctx* ctx, void* workspace_dev, size_t bytes, void* stream) {
+  if (!ctx) return MSPCG_EINVAL;
+  if (!ctx->configured) return fail(ctx, MSPCG_EINVAL, "call mspcg_workspace_bytes first");
+  if (!workspace_dev || bytes < ctx->ws_bytes || ((uintptr_t)workspace_dev & 255)) return fail(ctx, MSPCG_EINVAL, "workspace too small or misaligned");
+  cudaStream_t st = (cudaStream_t)stream;
+  Arena a; a.base = (char*)workspace_dev; a.cap = bytes;
+  carve(ctx, a);
+  const Lattice& L = ctx->lat;
+  CUDA_OK(ctx, up(ctx->gfull.nbrE, L.full.nbrE, st)); CUDA_OK(ctx, up(ctx->gfull.nbrO, L.full.nbrO, st));
+  CUDA_OK(ctx, up(ctx->gfull.cE, L.full.cE, st)); CUDA_OK(ctx, up(ctx->gfull.cO, L.full.cO, st));
+  CUDA_OK(ctx, up(ctx->gfull.origin, L.full.origin, st));
+  CUDA_OK(ctx, up(ctx->gblk.nbrE, L.blk.nbrE, st)); CUDA_OK(ctx, up(ctx->gblk.nbrO, L.blk.nbrO, st));
+  CUDA_OK(ctx, up(ctx->gblk.cE, L.blk.cE, st)); CUDA_OK(ctx, up(ctx->gblk.cO, L.blk.cO, st));
+  CUDA_OK(ctx, up(ctx->gblk.origin, L.blk.origin, st));
+  CUDA_OK(ctx, up(ctx->e_int_to_cb, L.e_int_to_cb, st));
+  CUDA_OK(ctx, cudaStreamSynchronize(st));
+  CUDA_OK(ctx, upload_mats<double>(ctx->md, ctx->hm, st)); CUDA_OK(ctx, upload_mats<float>(ctx->mf32, ctx->hm, st));
+  if (!ctx->sc_host) CUDA_OK(ctx, cudaMallocHost(&ctx->sc_host, sizeof(double) * 16));
+  ctx->have_ws = true;
+  return MSPCG_OK;
+}
+
+int mspcg_load_gauge(mspcg_ctx* ctx, const double* U_dev, int t_boundary, void* stream) {
+  int rc = check_ready(ctx, false); if (rc) return rc;
+  if (!U_dev || (t_boundary != 1 && t_boundary != -1)) return fail(ctx, MSPCG_EINVAL, "bad gauge pointer or t_boundary");
+  cudaStream_t st = (cudaStream_t)stream;
+  CUDA_OK(ctx, build_links_any(ctx, U_dev, ctx->full64, ctx->lat.full, ctx->gfull, t_boundary, st));
+  if (ctx->fullS.have) CUDA_OK(ctx, build_links_any(ctx, U_dev, ctx->fullS, ctx->lat.full, ctx->gfull, t_boundary, st));
+  CUDA_OK(ctx, build_links_any(ctx, U_dev, ctx->blkI, ctx->lat.blk, ctx->gblk, t_boundary, st));
+  ctx->have_gauge = true;
+  return MSPCG_OK;
+}
+
+size_t mspcg_vec_bytes(const mspcg_ctx* ctx, int prec) { return (ctx && prec_ok(prec)) ? vec_bytes(ctx, prec, ctx->Ls) : 0; }
+
+int mspcg_pack(mspcg_ctx* ctx, const double* abi_dev, void* native_dev, int prec, void* stream) {
+  int rc = check_ready(ctx, false); if (rc) return rc;
+  if (!abi_dev || !native_dev || !prec_ok(prec)) return fail(ctx, MSPCG_EINVAL, "bad argument");
+  CUDA_OK(ctx, pack_any(ctx, abi_dev, native_dev, prec, 1, (cudaStream_t)stream));
+  return MSPCG_OK;
+}
+int mspcg_unpack(mspcg_ctx* ctx, const void* native_dev, double* abi_dev, int prec, void* stream) {
+  int rc = check_ready(ctx, false); if (rc) return rc;
+  if (!abi_dev || !native_dev || !prec_ok(prec)) return fail(ctx, MSPCG_EINVAL, "bad argument");
+  CUDA_OK(ctx, pack_any(ctx, abi_dev, const_cast<void*>(native_dev), prec, 0, (cudaStream_t)stream));
+  return MSPCG_OK;
+}
+
+int mspcg_apply_MdagM(mspcg_ctx* ctx, const void* in_dev, void* out_dev, int prec, int layout, void* stream) {
+  int rc = check_ready(ctx, true); if (rc) return rc;
+  if (!in_dev || !out_dev || in_dev == out_dev || !full_buf(ctx, prec)) return fail(ctx, MSPCG_EINVAL, "bad pointer, aliasing, or precision not configured");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (layout == MSPCG_LAYOUT_NATIVE) {
+    CUDA_OK(ctx, normal_full_any(ctx, prec, in_dev, out_dev, nullptr, st));
+  } else {
+    CUDA_OK(ctx, pack_any(ctx, (const double*)in_dev, ctx->stage_in, prec, 1, st));
+    CUDA_OK(ctx, normal_full_any(ctx, prec, ctx->stage_in, ctx->stage_out, nullptr, st));
+    CUDA_OK(ctx, pack_any(ctx, (double*)out_dev, ctx->stage_out, prec, 0, st));
+  }
+  return MSPCG_OK;
+}
+
+int mspcg_apply_precond(mspcg_ctx* ctx, const void* r_dev, void* z_dev, int io_prec, int layout, int n_inner,
+                        int use_reduced, void* stream) {
+  int rc = check_ready(ctx, true); if (rc) return rc;
+  if (!r_dev || !z_dev || n_inner < 1 || n_inner > KMAX || !prec_ok(io_prec)) return fail(ctx, MSPCG_EINVAL, "bad argument (1 <= n_inner <= %d)", KMAX);
+  if (use_reduced) return fail(ctx, MSPCG_EINVAL, "reduced-Ls apply is not built yet (SURVEY 8(a) A10)");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (layout == MSPCG_LAYOUT_NATIVE) {
+    CUDA_OK(ctx, precond_any(ctx, r_dev, z_dev, io_prec, n_inner, st));
+  } else {
+    CUDA_OK(ctx, pack_any(ctx, (const double*)r_dev, ctx->stage_in, io_prec, 1, st));
+    CUDA_OK(ctx, precond_any(ctx, ctx->stage_in, ctx->stage_out, io_prec, n_inner, st));
+    CUDA_OK(ctx, pack_any(ctx, (double*)z_dev, ctx->stage_out, io_prec, 0, st));
+  }
+  return MSPCG_OK;
+}
+
+int mspcg_apply_MdagM_host(mspcg_ctx* ctx, const double* in_host, double* out_host, int prec) {
+  int rc = check_ready(ctx, true); if (rc) return rc;
+  const size_t n = vec_bytes(ctx, MSPCG_F64, ctx->Ls);
+  CUDA_OK(ctx, cudaMemcpyAsync(ctx->abi_in, in_host, n, cudaMemcpyHostToDevice, 0));
+  rc = mspcg_apply_MdagM(ctx, ctx->abi_in, ctx->abi_out, prec, MSPCG_LAYOUT_ABI, nullptr); if (rc) return rc;
+  CUDA_OK(ctx, cudaMemcpyAsync(out_host, ctx->abi_out, n, cudaMemcpyDeviceToHost, 0));
+  CUDA_OK(ctx, cudaStreamSynchronize(0));
+  return MSPCG_OK;
+}
+int mspcg_apply_precond_host(mspcg_ctx* ctx, const double* r_host, double* z_host, int io_prec, int n_inner, int use_reduced) {
+  int rc = check_ready(ctx, true); if (rc) return rc;
+  const size_t n = vec_bytes(ctx, MSPCG_F64, ctx->Ls);
+  CUDA_OK(ctx, cudaMemcpyAsync(ctx->abi_in, r_host, n, cudaMemcpyHostToDevice, 0));
+  rc = mspcg_apply_precond(ctx, ctx->abi_in, ctx->abi_out, io_prec, MSPCG_LAYOUT_ABI, n_inner, use_reduced, nullptr); if (rc) return rc;
+  CUDA_OK(ctx, cudaMemcpyAsync(z_host, ctx->abi_out, n, cudaMemcpyDeviceToHost, 0));
+  CUDA_OK(ctx, cudaStreamSynchronize(0));
+  return MSPCG_OK;
+}
+
+int mspcg_apply_A_block(mspcg_ctx* ctx, const double* in_dev, double* out_dev, int block, int prec, void* stream) {
+  int rc = check_ready(ctx, true); if (rc) return rc;
+  if (!in_dev || !out_dev || block < 0 || block >= ctx->lat.nblk || prec != ctx->inner_prec) return fail(ctx, MSPCG_EINVAL, "bad argument (prec must be the configured inner_prec)");
+  cudaStream_t st = (cudaStream_t)stream;
+  const Geometry& g = ctx->lat.blk;
+  const size_t blk_bytes = (size_t)g.nE0 * ctx->Ls * 24 * prec;
+  CUDA_OK(ctx, pack_any(ctx, in_dev, ctx->stage_in, prec, 1, st));
+  CUDA_OK(ctx, cudaMemsetAsync(ctx->stage_out, 0, vec_bytes(ctx, prec, ctx->Ls), st));
+  const char* pin = (const char*)ctx->stage_in + blk_bytes * block;
+  char* pout = (char*)ctx->stage_out + blk_bytes * block;
+#define AB(TT) { OpView<TT> v = one_block(make_view<TT>(ctx, ctx->blkI, g, ctx->gblk, ctx->Ls, false), block); \
+    DISPATCH_LS(ctx->Ls, CUDA_OK(ctx, (apply_normal<TT, LS>(ctx, v, mphi_plain<TT>((const TT*)pin), (const TT*)pin, (TT*)pout, nullptr, st)))); }
+  if (prec == MSPCG_F64) AB(double) else if (prec == MSPCG_F32) AB(float) else AB(__half)
+#undef AB
+  CUDA_OK(ctx, pack_any(ctx, out_dev, ctx->stage_out, prec, 0, st));
+  return MSPCG_OK;
+}
+
+int mspcg_solve(mspcg_ctx* ctx, const double* b_dev, double* x_dev, const mspcg_solve_params* params,
+                mspcg_solve_stats* stats, void* stream) {
+  int rc = check_ready(ctx, true); if (rc) return rc;
+  if (!b_dev || !x_dev || !params || !stats) return fail(ctx, MSPCG_EINVAL, "null argument");
+  if (params->use_precond && (params->n_inner < 1 || params->n_inner > KMAX)) return fail(ctx, MSPCG_EINVAL, "bad n_inner");
+  if (params->use_reduced_ls) return fail(ctx, MSPCG_EINVAL, "reduced-Ls apply is not built yet (SURVEY 8(a) A10)");
+  if (!full_buf(ctx, params->sloppy_prec)) return fail(ctx, MSPCG_EINVAL, "sloppy_prec not configured");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (params->sloppy_prec == MSPCG_F64) return solve_impl<double>(ctx, b_dev, x_dev, params, stats, st);
+  if (params->sloppy_prec == MSPCG_F32) return solve_impl<float>(ctx, b_dev, x_dev, params, stats, st);
+  return solve_impl<__half>(ctx, b_dev, x_dev, params, stats, st);
+}
+
+long mspcg_launch_count(const mspcg_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,209 @@
+"""GPU parity tests: the CUDA library (through its C ABI) against the CPU oracle, element by element, same seeded inputs.
+
+Tolerances (BASELINE.json north_star):
+  operator apply   rel-L2 <= 1e-12 (fp64), <= 1e-5 (fp32), <= 2e-3 (fp16 storage / fp32 arithmetic)
+  M_pre apply      rel-L2 <= 1e-9 (fp64, k <= 8: CG amplifies summation-order differences), 2e-2 (fp16)
+  solve            true fp64 residual <= 1e-10, solution within 1e-8 (relative) of the oracle's
+"""
+import numpy as np
+import pytest
+
+from oracle.cbind import OracleC
+from paper_2104_05615_b200 import F16, F32, F64, LAYOUT_NATIVE, Mspcg, synth
+
+pytestmark = pytest.mark.gpu
+
+MOB = dict(b=1.5, c=0.5, M5=1.8)
+
+
+def rel(a, b):
+    a = np.asarray(a, dtype=np.float64).reshape(-1)
+    b = np.asarray(b, dtype=np.float64).reshape(-1)
+    return np.linalg.norm(a - b) / np.linalg.norm(b)
+
+
+def setup(dims, Ls, mf, block, eps=0.3, gauge_seed=5, outer=F64, inner=F64, recon=18, tb=-1):
+    import torch
+    U = synth.gauge_natural_to_abi(synth.random_su3_links(dims, eps, gauge_seed), dims)
+    ora = OracleC(dims, Ls, MOB["b"], MOB["c"], MOB["M5"], mf, block)
+    ora.load_gauge(U, tb)
+    g = Mspcg(dims, Ls, MOB["b"], MOB["c"], MOB["M5"], mf, block)
+    g.configure(outer, inner, recon)
+    g.load_gauge(U, tb)
+    return ora, g, torch
+
+
+def dev(torch, a):
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64).reshape(-1)).cuda()
+
+
+# lattice, Ls, block: several thread-block tiles, ragged tails (site counts not multiples of the 8/16/32-site tile),
+# an uncut direction, blocks touching the antiperiodic boundary, and the wrap-around case L - B < 4 (PAD != PS, R10).
+GEOMS = [
+    ((4, 4, 4, 4), 8, (2, 2, 2, 2)),      # C1 geometry
+    ((2, 4, 6, 6), 4, (2, 2, 6, 2)),      # ragged, y partially cut, z uncut
+    ((8, 4, 4, 6), 6, (4, 4, 2, 6)),      # t uncut
+    ((4, 4, 4, 8), 12, (4, 2, 4, 4)),
+    ((4, 6, 4, 4), 16, (2, 6, 2, 2)),
+]
+
+
+def test_pack_unpack_roundtrip():
+    ora, g, torch = setup((4, 4, 6, 2), 6, 0.01, (2, 2, 2, 2))
+    v = synth.gaussian_spinor_abi((4, 4, 6, 2), 6, 3)
+    d = dev(torch, v)
+    for prec, tol in ((F64, 0.0), (F32, 1e-7), (F16, 1e-3)):
+        back = g.unpack(g.pack(d, prec), prec).cpu().numpy()
+        assert rel(back, v) <= tol
+
+
+@pytest.mark.parametrize("dims,Ls,block", GEOMS)
+def test_MdagM_fp64(dims, Ls, block):
+    ora, g, torch = setup(dims, Ls, 0.02, block)
+    v = synth.gaussian_spinor_abi(dims, Ls, 7)
+    out = g.apply_MdagM(dev(torch, v), F64).cpu().numpy()
+    assert rel(out, ora.apply_MdagM(v)) <= 1e-12
+
+
+@pytest.mark.parametrize("tb", [+1, -1])
+def test_MdagM_fp64_boundary_and_unit_gauge(tb):
+    import torch
+    dims, Ls = (4, 4, 4, 6), 8
+    U = synth.gauge_natural_to_abi(synth.unit_links(dims), dims)
+    ora = OracleC(dims, Ls, MOB["b"], MOB["c"], MOB["M5"], 0.05, dims)
+    ora.load_gauge(U, tb)
+    g = Mspcg(dims, Ls, MOB["b"], MOB["c"], MOB["M5"], 0.05, dims)
+    g.configure(F64, F64, 18)
+    g.load_gauge(U, tb)
+    v = synth.gaussian_spinor_abi(dims, Ls, 8)
+    assert rel(g.apply_MdagM(dev(torch, v), F64).cpu().numpy(), ora.apply_MdagM(v)) <= 1e-12
+
+
+@pytest.mark.parametrize("prec,tol,recon", [(F32, 1e-5, 18), (F16, 2e-3, 18), (F32, 1e-5, 12), (F16, 2e-3, 12)])
+def test_MdagM_low_precision(prec, tol, recon):
+    dims, Ls, block = (4, 4, 6, 8), 8, (2, 2, 6, 4)
+    ora, g, torch = setup(dims, Ls, 0.02, block, outer=prec, inner=prec, recon=recon)
+    v = synth.gaussian_spinor_abi(dims, Ls, 9)
+    ref = ora.apply_MdagM(v)
+    d = dev(torch, v)
+    assert rel(g.apply_MdagM(d, prec).cpu().numpy(), ref) <= tol
+    nat = g.pack(d, prec)
+    out = g.unpack(g.apply_MdagM(nat, prec, LAYOUT_NATIVE), prec).cpu().numpy()
+    assert rel(out, ref) <= tol
+
+
+@pytest.mark.parametrize("dims,Ls,block", GEOMS)
+def test_A_block_fp64(dims, Ls, block):
+    ora, g, torch = setup(dims, Ls, 0.02, block)
+    v = synth.gaussian_spinor_abi(dims, Ls, 11)
+    d = dev(torch, v)
+    nblk = g.geometry()["nblk"]
+    assert nblk == ora.num_blocks
+    for blk in sorted({0, nblk // 2, nblk - 1}):
+        out = g.apply_A_block(d, blk, F64).cpu().numpy()
+        assert rel(out, ora.apply_A_block(v, blk)) <= 1e-12
+
+
+@pytest.mark.parametrize("dims,Ls,block", GEOMS)
+@pytest.mark.parametrize("k", [1, 4])
+def test_precond_fp64(dims, Ls, block, k):
+    ora, g, torch = setup(dims, Ls, 0.02, block)
+    r = synth.gaussian_spinor_abi(dims, Ls, 13)
+    z = g.apply_precond(dev(torch, r), k, F64).cpu().numpy()
+    assert rel(z, ora.apply_precond(r, k)) <= 1e-9
+
+
+def test_precond_degenerate_inputs():
+    dims, Ls, block = (4, 4, 4, 4), 8, (2, 2, 2, 2)
+    ora, g, torch = setup(dims, Ls, 0.02, block)
+    r = synth.gaussian_spinor_abi(dims, Ls, 14)
+    # zero right-hand side -> zero, never NaN (R13)
+    z0 = g.apply_precond(dev(torch, 0 * r), 6, F64).cpu().numpy()
+    assert np.all(z0 == 0.0)
+    # one block's right-hand side zero: that block returns zero, the others are untouched (block independence)
+    rr = r.copy()
+    mask = ora.apply_A_block(np.ones_like(r), 5) != 0  # support of block 5
+    rr[mask] = 0.0
+    z = g.apply_precond(dev(torch, rr), 4, F64).cpu().numpy().reshape(r.shape)
+    zr = ora.apply_precond(rr, 4).reshape(r.shape)
+    assert np.all(z[mask] == 0.0) and rel(z, zr) <= 1e-9
+    # scale equivariance z(lambda r) = lambda z(r)
+    z1 = g.apply_precond(dev(torch, r), 3, F64).cpu().numpy()
+    z2 = g.apply_precond(dev(torch, 1e-7 * r), 3, F64).cpu().numpy()
+    assert rel(z2 * 1e7, z1) <= 1e-10
+    # k >> dimension of the Krylov space that matters: many iterations stay finite
+    zk = g.apply_precond(dev(torch, r), 32, F64).cpu().numpy()
+    assert np.all(np.isfinite(zk))
+
+
+@pytest.mark.parametrize("inner,tol", [(F32, 2e-4), (F16, 2e-2)])
+def test_precond_low_precision(inner, tol):
+    dims, Ls, block = (4, 4, 8, 8), 8, (4, 4, 4, 4)
+    ora, g, torch = setup(dims, Ls, 0.02, block, outer=F32, inner=inner)
+    r = synth.gaussian_spinor_abi(dims, Ls, 15)
+    ref = ora.apply_precond(r, 6)
+    z = g.apply_precond(dev(torch, r), 6, F64).cpu().numpy()
+    assert rel(z, ref) <= tol
+    # tiny right-hand side: the per-block rescaling keeps fp16 in range (R14)
+    z = g.apply_precond(dev(torch, 1e-9 * r), 6, F64).cpu().numpy()
+    assert rel(z * 1e9, ref) <= tol
+
+
+def test_solve_C1_cg_and_mspcg_fp64():
+    """BASELINE.json configs[0]: 4^4, Ls 8, mf 0.01, 2^4 blocks, 6 inner iterations, tol 1e-10."""
+    cfg = synth.CONFIGS["C1"]
+    dims, Ls, block = cfg["dims"], cfg["Ls"], cfg["block"]
+    ora, g, torch = setup(dims, Ls, cfg["mf"], block, eps=cfg["eps"], gauge_seed=cfg["gauge_seed"])
+    b = synth.gaussian_spinor_abi(dims, Ls, cfg["src_seed"])
+    x_ora, so = ora.solve(b, tol=1e-10, use_precond=False)
+    x_orap, sop = ora.solve(b, tol=1e-10, use_precond=True, n_inner=cfg["n_inner"])
+    db = dev(torch, b)
+    x, s = g.solve(db, tol=1e-10, use_precond=False)
+    xp, spc = g.solve(db, tol=1e-10, use_precond=True, n_inner=cfg["n_inner"])
+    for xx, ss in ((x, s), (xp, spc)):
+        assert ss["rc"] == 0 and ss["converged"] == 1
+        assert ss["true_res"] <= 1e-10
+        # independent check of the residual with the oracle's operator
+        xn = xx.cpu().numpy()
+        assert rel(ora.apply_MdagM(xn), b) <= 1e-10 * 1.01
+        assert rel(xn, x_ora) <= 1e-8
+    assert rel(x_orap, x_ora) <= 1e-8
+    assert abs(s["iters"] - so["iters"]) <= 3
+    assert abs(spc["iters"] - sop["iters"]) <= 3
+    assert spc["iters"] < s["iters"]
+    assert spc["inner_applies"] > 0
+
+
+def test_solve_mixed_precision_reliable_updates():
+    dims, Ls, block = (4, 4, 4, 8), 8, (2, 2, 2, 4)
+    ora, g, torch = setup(dims, Ls, 0.01, block, eps=0.3, outer=F32, inner=F16)
+    b = synth.gaussian_spinor_abi(dims, Ls, 17)
+    x_ora, _ = ora.solve(b, tol=1e-11, use_precond=False)
+    db = dev(torch, b)
+    for pre in (False, True):
+        x, s = g.solve(db, tol=1e-10, use_precond=pre, n_inner=5, sloppy_prec=F32, delta=0.1)
+        assert s["rc"] == 0 and s["true_res"] <= 1e-10 and s["reliable_updates"] >= 2
+        assert rel(x.cpu().numpy(), x_ora) <= 1e-8
+    # zero right-hand side and a non-zero initial guess
+    x, s = g.solve(0 * db, tol=1e-10)
+    assert s["converged"] == 1 and s["iters"] == 0 and float(x.abs().max()) == 0.0
+    x, s = g.solve(db, x0_abi=dev(torch, x_ora), tol=1e-10)
+    assert s["converged"] == 1 and s["iters"] <= 1
+
+
+def test_error_codes():
+    import torch
+    g = Mspcg((4, 4, 4, 4), 8, 1.5, 0.5, 1.8, 0.01, (2, 2, 2, 2))
+    v = torch.zeros(g.nreal, dtype=torch.float64, device="cuda")
+    from paper_2104_05615_b200 import MspcgError
+    with pytest.raises(MspcgError) as e:
+        g.apply_MdagM(v, F64)
+    assert e.value.code == -7  # no workspace
+    g.configure(F64, F64, 18)
+    with pytest.raises(MspcgError) as e:
+        g.apply_MdagM(v, F64)
+    assert e.value.code == -4  # no gauge
+    with pytest.raises(MspcgError):
+        Mspcg((4, 4, 4, 5), 8, 1.5, 0.5, 1.8, 0.01)
+    with pytest.raises(MspcgError):
+        Mspcg((4, 4, 4, 4), 8, 1.5, 0.5, 1.8, 0.01, (3, 2, 2, 2))
