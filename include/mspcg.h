@@ -131,6 +131,15 @@ int mspcg_solve(mspcg_ctx* ctx, const double* b_dev, double* x_dev, const mspcg_
 /* Counters for reports: kernels launched by this context since creation. */
 long mspcg_launch_count(const mspcg_ctx* ctx);
 
+/* Per-kernel device timing for roofline reports.  mspcg_timing(ctx, 1) makes every later launch of the operator
+ * kernels record a CUDA-event pair on its stream; mspcg_timing_read synchronises the device, sums the elapsed
+ * milliseconds and launch counts per class into ms_host[10], launches_host[10] (HOST) and clears the record.
+ * class = 5*geometry + kind;  geometry 0 = whole lattice, 1 = Dirichlet blocks;  kind 0 = Mphi (kernel 1 of eq. 16),
+ * 1 = fused hop with one 5D matrix (kernels 2 and 4), 2 = fused hop of kernel 3, 3 = fused hop of kernel 5 (+dot),
+ * 4 = BLAS-1 of the inner CG.  Off by default; timed benchmark regions run with it off. */
+int mspcg_timing(mspcg_ctx* ctx, int enable);
+int mspcg_timing_read(mspcg_ctx* ctx, double* ms_host, long* launches_host);
+
 #ifdef __cplusplus
 }
 #endif

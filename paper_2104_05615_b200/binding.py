@@ -23,6 +23,7 @@ SYMBOLS = [
     "mspcg_workspace_bytes", "mspcg_set_workspace", "mspcg_load_gauge", "mspcg_vec_bytes", "mspcg_pack",
     "mspcg_unpack", "mspcg_apply_MdagM", "mspcg_apply_precond", "mspcg_apply_MdagM_host",
     "mspcg_apply_precond_host", "mspcg_apply_A_block", "mspcg_set_reduced_ls", "mspcg_solve", "mspcg_launch_count",
+    "mspcg_timing", "mspcg_timing_read",
 ]
 
 
@@ -72,6 +73,8 @@ def load_library():
     L.mspcg_solve.argtypes = [vp, vp, vp, C.POINTER(SolveParams), C.POINTER(SolveStats), vp]
     L.mspcg_launch_count.argtypes = [vp]
     L.mspcg_launch_count.restype = C.c_long
+    L.mspcg_timing.argtypes = [vp, i]
+    L.mspcg_timing_read.argtypes = [vp, dp, C.POINTER(C.c_long)]
     _lib = L
     return L
 
@@ -235,3 +238,15 @@ class Mspcg:
 
     def launch_count(self):
         return int(self.lib.mspcg_launch_count(self.h))
+
+    TIMING_CLASSES = ["full.mphi", "full.hop_k2k4", "full.hop_k3", "full.hop_k5", "full.blas",
+                      "blk.mphi", "blk.hop_k2k4", "blk.hop_k3", "blk.hop_k5", "blk.blas"]
+
+    def timing(self, enable):
+        self._check(self.lib.mspcg_timing(self.h, int(bool(enable))))
+
+    def timing_read(self):
+        ms = (C.c_double * 10)()
+        n = (C.c_long * 10)()
+        self._check(self.lib.mspcg_timing_read(self.h, ms, n))
+        return {k: dict(ms=ms[j], launches=n[j]) for j, k in enumerate(self.TIMING_CLASSES)}

@@ -58,6 +58,9 @@ struct mspcg_ctx {
   std::vector<double> T_host;
   std::string err;
   long launches = 0;
+  // optional per-launch CUDA-event timing (mspcg_timing): class = geometry*5 + kind
+  bool timing = false; int cur_geom = 0;
+  std::vector<cudaEvent_t> ev_pool; std::vector<int> ev_cls; size_t ev_used = 0;
   // configuration
   int outer_prec = 0, inner_prec = 0, recon = 18;
   bool configured = false, have_ws = false, have_gauge = false;
@@ -153,6 +156,19 @@ void carve(mspcg_ctx* c, Arena& a) {
   c->abi_in = (double*)a.take_bytes(n64); c->abi_out = (double*)a.take_bytes(n64);
 }
 
+// ------------------------------------------------------------------------------------------------ per-launch timing
+enum { KIND_MPHI = 0, KIND_HOP_PLAIN = 1, KIND_HOP_K3 = 2, KIND_HOP_XPAY = 3, KIND_BLAS = 4, NKIND = 5, NCLASS = 10 };
+struct TimedLaunch {   // records an event pair around one launch when timing is on
+  mspcg_ctx* c; cudaStream_t st; bool on;
+  TimedLaunch(mspcg_ctx* c_, int kind, cudaStream_t st_) : c(c_), st(st_), on(c_->timing) {
+    if (!on) return;
+    if (c->ev_used + 2 > c->ev_pool.size()) { cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b); c->ev_pool.push_back(a); c->ev_pool.push_back(b); }
+    c->ev_cls.push_back(c->cur_geom * NKIND + kind);
+    cudaEventRecord(c->ev_pool[c->ev_used], st);
+  }
+  ~TimedLaunch() { if (on) { cudaEventRecord(c->ev_pool[c->ev_used + 1], st); c->ev_used += 2; } }
+};
+
 // ------------------------------------------------------------------------------------------------ kernel launchers
 #define DISPATCH_LS(LSV, ...)                                            \
   switch (LSV) {                                                         \
@@ -173,7 +189,8 @@ cudaError_t launch_hop(mspcg_ctx* c, const HopArgs<T>& a, int nblk, cudaStream_t
   const size_t sm = hop_smem<T, LS, EPI>();
   if (!attr) { cudaFuncSetAttribute(k_hop<T, LS, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); attr = true; }
   dim3 block(LS, Tile<LS>::NS), grid((a.n_out + Tile<LS>::NS - 1) / Tile<LS>::NS, nblk);
-  k_hop<T, LS, EPI><<<grid, block, sm, st>>>(a);
+  { TimedLaunch tl(c, EPI == EPI_PLAIN ? KIND_HOP_PLAIN : (EPI == EPI_K3 ? KIND_HOP_K3 : KIND_HOP_XPAY), st);
+    k_hop<T, LS, EPI><<<grid, block, sm, st>>>(a); }
   c->launches++;
   return cudaPeekAtLastError();
 }
@@ -184,7 +201,7 @@ cudaError_t launch_mphi(mspcg_ctx* c, const MphiArgs<T>& a, int nblk, cudaStream
   const size_t sm = sizeof(C) * (size_t)SM::NS * SM::SSTRIDE;
   if (!attr) { cudaFuncSetAttribute(k_mphi<T, LS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); attr = true; }
   dim3 block(LS, Tile<LS>::NS), grid((unsigned)((a.n_sites + Tile<LS>::NS - 1) / Tile<LS>::NS), nblk);
-  k_mphi<T, LS><<<grid, block, sm, st>>>(a);
+  { TimedLaunch tl(c, KIND_MPHI, st); k_mphi<T, LS><<<grid, block, sm, st>>>(a); }
   c->launches++;
   return cudaPeekAtLastError();
 }
@@ -279,25 +296,27 @@ cudaError_t precond_impl(mspcg_ctx* c, const TIO* r_in, TIO* z_out, int k, cudaS
   const Geometry& g = c->lat.blk;
   const int nblk = g.nblk;
   OpView<T> v = make_view<T>(c, c->blkI, g, c->gblk, LS, false);
+  c->cur_geom = 1;
   cudaError_t e;
   if ((e = cudaMemsetAsync(c->rho, 0, sizeof(double) * (size_t)(KMAX + 1) * nblk, st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(c->pq, 0, sizeof(double) * (size_t)KMAX * nblk, st)) != cudaSuccess) return e;
   const float* scale = nullptr;
   if (sizeof(T) == 2) {   // fp16 storage: rescale every block's right-hand side to max-abs 1 (R14)
     if ((e = cudaMemsetAsync(c->scale, 0, sizeof(float) * nblk, st)) != cudaSuccess) return e;
-    k_maxabs<TIO><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(r_in, g.nE0, LS, c->scale);
+    { TimedLaunch tl(c, KIND_BLAS, st); k_maxabs<TIO><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(r_in, g.nE0, LS, c->scale); }
     c->launches++;
     scale = c->scale;
   }
   T *r = (T*)c->in_r, *p = (T*)c->in_p, *q = (T*)c->in_q; TX* x = (TX*)c->in_x;
-  k_pre_begin<TIO, T><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(r_in, r, g.nE0, LS, scale, c->rho);
+  { TimedLaunch tl(c, KIND_BLAS, st); k_pre_begin<TIO, T><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(r_in, r, g.nE0, LS, scale, c->rho); }
   c->launches++;
   for (int it = 0; it < k; it++) {
     MphiArgs<T> mp; memset(&mp, 0, sizeof(mp));
     mp.in = r; mp.p = p; mp.mode = 2; mp.it = it; mp.nblk = nblk; mp.rho = c->rho; mp.pq = c->pq;
     if ((e = apply_normal<T, LS>(c, v, mp, p, q, c->pq + (size_t)it * nblk, st)) != cudaSuccess) return e;
-    k_inner_update<T, TX, TIO><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(p, q, r, x, z_out, g.nE0, LS, it, nblk, it == k - 1,
-                                                                          c->rho, c->pq, scale);
+    { TimedLaunch tl(c, KIND_BLAS, st);
+      k_inner_update<T, TX, TIO><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(p, q, r, x, z_out, g.nE0, LS, it, nblk, it == k - 1,
+                                                                            c->rho, c->pq, scale); }
     c->launches++;
   }
   return cudaPeekAtLastError();
@@ -323,6 +342,7 @@ cudaError_t precond_any(mspcg_ctx* c, const void* r, void* z, int io_prec, int k
 template <typename T>
 cudaError_t normal_full(mspcg_ctx* c, const OpBuf& ob, const T* p, T* q, MphiArgs<T> mp, double* dot_out, cudaStream_t st) {
   OpView<T> v = make_view<T>(c, ob, c->lat.full, c->gfull, c->Ls, false);
+  c->cur_geom = 0;
   DISPATCH_LS(c->Ls, return (apply_normal<T, LS>(c, v, mp, p, q, dot_out, st)));
   return cudaErrorInvalidValue;
 }
@@ -547,6 +567,7 @@ int mspcg_create(mspcg_ctx** out, int Lx, int Ly, int Lz, int Lt, int Ls, double
 int mspcg_destroy(mspcg_ctx* ctx) {
   if (!ctx) return MSPCG_EINVAL;
   if (ctx->sc_host) cudaFreeHost(ctx->sc_host);
+  for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
   delete ctx;
   return MSPCG_OK;
 }
@@ -695,6 +716,7 @@ int mspcg_apply_A_block(mspcg_ctx* ctx, const double* in_dev, double* out_dev, i
   CUDA_OK(ctx, cudaMemsetAsync(ctx->stage_out, 0, vec_bytes(ctx, prec, ctx->Ls), st));
   const char* pin = (const char*)ctx->stage_in + blk_bytes * block;
   char* pout = (char*)ctx->stage_out + blk_bytes * block;
+  ctx->cur_geom = 1;
 #define AB(TT) { OpView<TT> v = one_block(make_view<TT>(ctx, ctx->blkI, g, ctx->gblk, ctx->Ls, false), block); \
     DISPATCH_LS(ctx->Ls, CUDA_OK(ctx, (apply_normal<TT, LS>(ctx, v, mphi_plain<TT>((const TT*)pin), (const TT*)pin, (TT*)pout, nullptr, st)))); }
   if (prec == MSPCG_F64) AB(double) else if (prec == MSPCG_F32) AB(float) else AB(__half)
@@ -717,5 +739,24 @@ int mspcg_solve(mspcg_ctx* ctx, const double* b_dev, double* x_dev, const mspcg_
 }
 
 long mspcg_launch_count(const mspcg_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int mspcg_timing(mspcg_ctx* ctx, int enable) {
+  if (!ctx) return MSPCG_EINVAL;
+  ctx->timing = enable != 0; ctx->ev_used = 0; ctx->ev_cls.clear();
+  return MSPCG_OK;
+}
+
+int mspcg_timing_read(mspcg_ctx* ctx, double* ms_host, long* launches_host) {
+  if (!ctx || !ms_host || !launches_host) return MSPCG_EINVAL;
+  for (int i = 0; i < NCLASS; i++) { ms_host[i] = 0; launches_host[i] = 0; }
+  CUDA_OK(ctx, cudaDeviceSynchronize());
+  for (size_t i = 0; i < ctx->ev_cls.size(); i++) {
+    float ms = 0;
+    CUDA_OK(ctx, cudaEventElapsedTime(&ms, ctx->ev_pool[2 * i], ctx->ev_pool[2 * i + 1]));
+    ms_host[ctx->ev_cls[i]] += ms; launches_host[ctx->ev_cls[i]]++;
+  }
+  ctx->ev_used = 0; ctx->ev_cls.clear();
+  return MSPCG_OK;
+}
 
 }  // extern "C"
