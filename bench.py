@@ -1,0 +1,414 @@
+#!/usr/bin/env python
+"""bench.py -- B200 benchmark of the MSPCG hot path (BASELINE.json configs[1] = "C2", operator-only benchmark).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C2] [--no-extras]
+
+One "step" = one pass of the whole hot path over one batch of synthetic input = the operator work of one outer MSPCG
+iteration on the C2 lattice (16^3 x 32, Ls 16, 8^4 Dirichlet blocks):
+    one multi-splitting preconditioner application  z = M^-1 r  (6 inner CG iterations, fp16 storage / fp32
+    arithmetic, all 32 blocks batched)  +  one full-lattice D^dag D application in the sloppy
+    outer precision fp32 (A2-A6),
+both on NATIVE-layout vectors already resident in HBM.  value = GFLOP/s with the flop convention of SURVEY 8(d)
+(hop 1320, bidiagonal 5D op 72, xpay 48, dense 5D contraction 48*Ls per 5D site; halo-shell sites count as work).
+The JSON line also carries: e2e (same step through the C-ABI *_host calls, host<->device copies in the timed
+region), roofline (dominant kernel, algorithmic bytes / CUDA-event time vs the measured HBM peak), cpu_baseline (the
+CPU oracle on a bounded sample), clocks, and "extras" (per-precision operator numbers, CG vs MSPCG time-to-solution).
+
+Multi-GPU: the path does not shard (BASELINE.json: one GPU, no collectives) -> replicas only: under torchrun every
+rank runs the same workload on its own GPU, no data-path collective, value = sum over ranks / max time ("weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2104_05615_b200 import synth  # noqa: E402
+
+METRIC = "mspcg_precond_dslash_step_gflops"
+UNIT = "GFLOP/s"
+
+
+# ------------------------------------------------------------------------------------------------ work models
+def stage_sites(geo, full):
+    """4D sites per block on which each of the five kernels of eq. 16 writes: (K1, K2, K3, K4, K5)."""
+    if full:
+        v = geo["vh"]
+        return dict(nblk=1, nE0=v, nO=v, nE=v)
+    return dict(nblk=geo["nblk"], nE0=geo["nE0"], nO=geo["nO1"], nE=geo["nE2"])
+
+
+def flops_normal(st, Ls):
+    """Flops of one D^dag D (or A_s, all blocks) application; SURVEY 8(d) convention."""
+    hop, bid, xpay, dense = 1320, 72, 48, 48 * Ls
+    per_block = (bid * st["nE0"] + (hop + dense) * st["nO"] + (hop + 2 * dense + xpay) * st["nE"]
+                 + (hop + dense) * st["nO"] + (hop + bid + xpay) * st["nE0"]) * Ls
+    return per_block * st["nblk"]
+
+
+def bytes_normal(st, Ls, w, ng, fused_pupdate=False, with_dot=False):
+    """Algorithmic HBM bytes per kernel class of one D^dag D application: every input site, output site and link read
+    or written exactly once per kernel (ideal neighbour reuse).  Returns dict class -> bytes per launch."""
+    site = Ls * 24 * w
+    link = 8 * ng * w
+    n = st["nblk"]
+    k1 = (4 if fused_pupdate else 2) * st["nE0"] * site
+    k2 = (st["nE0"] + st["nO"]) * site + st["nO"] * link
+    k3 = (st["nO"] + st["nE0"] + st["nE"] + st["nE0"]) * site + st["nE"] * link
+    k4 = (st["nE"] + st["nO"]) * site + st["nO"] * link
+    k5 = (st["nO"] + st["nE0"] + (st["nE0"] if with_dot else 0) + st["nE0"]) * site + st["nE0"] * link
+    return dict(mphi=k1 * n, hop_k2=k2 * n, hop_k3=k3 * n, hop_k4=k4 * n, hop_k5=k5 * n)
+
+
+def precond_work(geo, Ls, k, w_in, w_io, ng):
+    """Flops and algorithmic bytes of one M^-1 application (k inner iterations)."""
+    st = stage_sites(geo, False)
+    fl = k * flops_normal(st, Ls)
+    by = 0
+    for it in range(k):
+        b = bytes_normal(st, Ls, w_in, ng, fused_pupdate=it > 0, with_dot=True)
+        if it == 0:
+            b["mphi"] = 3 * st["nE0"] * Ls * 24 * w_in * st["nblk"]
+        by += sum(b.values())
+        v = st["nE0"] * Ls * 24 * st["nblk"]
+        wx = 4 if w_in == 2 else w_in
+        by += v * (3 * w_in + 2 * wx + 2 * w_in) if it < k - 1 else v * (w_in + wx + w_io)   # x,r update / final z
+    by += st["nE0"] * Ls * 24 * st["nblk"] * (w_io * (2 if w_in == 2 else 1) + w_in)         # max-abs + scaled copy
+    return fl, by
+
+
+# ------------------------------------------------------------------------------------------------ clocks sampler
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except Exception:
+                continue
+            for nme, val in zip(names, r[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nme)
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    power_w_max=max(pw) if pw else None, samples=len(sm), reasons=sorted(reasons))
+
+
+# ------------------------------------------------------------------------------------------------ workload set-up
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic():
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture, if any."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    return json.load(open(p)) if os.path.exists(p) else {}
+
+
+def make_inputs(cfg):
+    dims, Ls = cfg["dims"], cfg["Ls"]
+    U = synth.gauge_natural_to_abi(synth.random_su3_links(dims, cfg["eps"], cfg["gauge_seed"]), dims)
+    src = synth.gaussian_spinor_abi(dims, Ls, cfg["src_seed"])
+    return U, src
+
+
+def timed(torch, fn, steps, warmup, barrier=None):
+    """W warm-up calls, then exactly K calls between CUDA events on the current stream; returns ms total."""
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+    return e0.elapsed_time(e1)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2104_05615_b200 import F16, F32, F64, LAYOUT_NATIVE, Mspcg
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    barrier = None
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        barrier = dist.barrier
+    cfg = synth.CONFIGS[args.workload]
+    dims, Ls, block, k = cfg["dims"], cfg["Ls"], cfg["block"], cfg["n_inner"]
+    U, src = make_inputs(cfg)
+    g = Mspcg(dims, Ls, cfg["b"], cfg["c"], cfg["M5"], cfg["mf"], block)
+    ws = g.configure(F32, F16, 18)
+    g.load_gauge(U, -1)
+    geo = g.geometry()
+    d_src = torch.as_tensor(src.reshape(-1)).cuda()
+    r32 = g.pack(d_src, F32)
+    z32, q32 = g.new_native(F32), g.new_native(F32)
+
+    def step():
+        g.apply_precond(r32, k, F32, LAYOUT_NATIVE, out=z32)
+        g.apply_MdagM(r32, F32, LAYOUT_NATIVE, out=q32)
+
+    # ---- work model of one step
+    fl_pre, by_pre = precond_work(geo, Ls, k, 2, 4, 18)
+    st_full = stage_sites(geo, True)
+    fl_op = flops_normal(st_full, Ls)
+    by_op = sum(bytes_normal(st_full, Ls, 4, 18).values())
+    flops_step = fl_pre + fl_op
+
+    # ---- the timed region (device-resident inputs)
+    sampler = ClockSampler(local)
+    sampler.start()
+    n0 = g.launch_count()
+    ms = timed(torch, step, args.steps, args.warmup, barrier)
+    launches = (g.launch_count() - n0) // (args.steps + args.warmup) * args.steps
+    clocks = sampler.stop()
+    if world > 1:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ms_step = ms / args.steps
+    value = world * flops_step / (ms_step * 1e-3) / 1e9
+
+    # ---- end to end: same step through the *_host entry points, pinned host buffers, copies inside the timed region
+    h_in = torch.as_tensor(src.reshape(-1)).pin_memory()
+    h_z, h_q = torch.empty_like(h_in).pin_memory(), torch.empty_like(h_in).pin_memory()
+
+    def step_host():
+        g.apply_precond_host(h_in, h_z, k, F32)
+        g.apply_MdagM_host(h_in, h_q, F32)
+
+    e2e_steps = max(2, min(args.steps, 5))
+    ms_e2e = timed(torch, step_host, e2e_steps, 1, barrier) / e2e_steps
+    if world > 1:
+        t = torch.tensor([ms_e2e], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t.item())
+    nb = h_in.numel() * 8
+    e2e = dict(value=world * flops_step / (ms_e2e * 1e-3) / 1e9, unit=UNIT, ms_per_step=ms_e2e,
+               h2d_bytes_per_step=2 * nb, d2h_bytes_per_step=2 * nb)
+
+    # ---- roofline of the dominant kernel: instrumented repetition of the same steps (CUDA events per launch)
+    peak, peak_src = peaks()
+    g.timing(True)
+    for _ in range(args.steps):
+        step()
+    tm = g.timing_read()
+    g.timing(False)
+    st_blk = stage_sites(geo, False)
+    bb = bytes_normal(st_blk, Ls, 2, 18, fused_pupdate=True, with_dot=True)
+    bf = bytes_normal(st_full, Ls, 4, 18)
+    alg = {"blk.hop_k2k4": 0.5 * (bb["hop_k2"] + bb["hop_k4"]), "blk.hop_k3": bb["hop_k3"], "blk.hop_k5": bb["hop_k5"],
+           "blk.mphi": bb["mphi"], "full.hop_k2k4": 0.5 * (bf["hop_k2"] + bf["hop_k4"]), "full.hop_k3": bf["hop_k3"],
+           "full.hop_k5": bf["hop_k5"], "full.mphi": bf["mphi"]}
+    kern = {}
+    tot_ms = sum(v["ms"] for v in tm.values())
+    for name, v in tm.items():
+        if v["launches"] == 0:
+            continue
+        avg = v["ms"] / v["launches"]
+        ent = dict(launches_per_step=v["launches"] / args.steps, avg_ms=avg, share=v["ms"] / tot_ms)
+        if name in alg:
+            ent["alg_bytes"] = alg[name]
+            ent["GBps"] = alg[name] / (avg * 1e-3) / 1e9
+            ent["frac"] = ent["GBps"] / peak
+        kern[name] = ent
+    dom = max((n for n in kern if n in alg), key=lambda n: tm[n]["ms"])
+    traffic = ncu_traffic().get(dom)
+    roofline = dict(bound="hbm", kernel=dom, achieved=kern[dom]["GBps"], peak=peak, unit="GB/s", frac=kern[dom]["frac"],
+                    traffic=traffic, peak_source=peak_src, alg_bytes_per_launch=kern[dom]["alg_bytes"],
+                    avg_launch_ms=kern[dom]["avg_ms"], share_of_step=kern[dom]["share"])
+
+    out = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+               ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f16/f32",
+               data="synthetic", impl="ours",
+               config=dict(workload=f"{args.workload}: {dims[0]}x{dims[1]}x{dims[2]}x{dims[3]} Ls={Ls} blocks {block} "
+                                    f"M_pre(k={k}, fp16 storage/fp32 math) + DdagD(fp32)", parallelism="replicas only",
+                           l2="working set of a step %.0f MiB > 126 MB L2 (no flush)" % (ws / 2**20), workspace_bytes=ws,
+                           flops_per_step=flops_step, alg_bytes_per_step=by_pre + by_op),
+               gpu_launches=launches, clocks=clocks, e2e=e2e, roofline=roofline, kernels=kern,
+               step_GBps_algorithmic=(by_pre + by_op) / (ms_step * 1e-3) / 1e9)
+    if rank == 0 and world == 1 and not args.no_extras:
+        out["extras"] = extras(torch, g, cfg, U, src, d_src, geo, peak, args)
+        out["cpu_baseline"] = cpu_baseline(cfg, U, src, geo)
+    if rank == 0:
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def extras(torch, g, cfg, U, src, d_src, geo, peak, args):
+    """Per-precision operator numbers (C2: "in fp16 storage with fp32 accumulation and in fp64") and CG vs MSPCG
+    time-to-solution on the same lattice.  Outside the headline timed region."""
+    from paper_2104_05615_b200 import F16, F32, F64, LAYOUT_NATIVE, Mspcg
+    dims, Ls, block, k = cfg["dims"], cfg["Ls"], cfg["block"], cfg["n_inner"]
+    st_full = stage_sites(geo, True)
+    ex = {}
+    steps, warm = max(3, args.steps), 3
+
+    def op_entry(ms, flops, nbytes):
+        return dict(ms=ms, GFLOPs=flops / (ms * 1e-3) / 1e9, GBps_algorithmic=nbytes / (ms * 1e-3) / 1e9,
+                    hbm_frac=nbytes / (ms * 1e-3) / 1e9 / peak)
+
+    def time_op(ctx, prec, w):
+        v, o = ctx.pack(d_src, prec), ctx.new_native(prec)
+        ms = timed(torch, lambda: ctx.apply_MdagM(v, prec, LAYOUT_NATIVE, out=o), steps, warm) / steps
+        return op_entry(ms, flops_normal(st_full, Ls), sum(bytes_normal(st_full, Ls, w, 18).values()))
+
+    def time_pre(ctx, io, w_in, w_io):
+        v, o = ctx.pack(d_src, io), ctx.new_native(io)
+        ms = timed(torch, lambda: ctx.apply_precond(v, k, io, LAYOUT_NATIVE, out=o), steps, warm) / steps
+        fl, by = precond_work(geo, Ls, k, w_in, w_io, 18)
+        return op_entry(ms, fl, by)
+
+    ex["DdagD_fp64"] = time_op(g, F64, 8)
+    ex["DdagD_fp32"] = time_op(g, F32, 4)
+    ex["Mpre_k%d_fp16_io32" % k] = time_pre(g, F32, 2, 4)
+    # time to solution, plain CG vs MSPCG, sloppy fp32 + fp64 reliable updates, preconditioner fp16
+    sol = {}
+    for name, pre in (("CG", False), ("MSPCG", True)):
+        x, s = g.solve(d_src, tol=1e-10, max_iter=20000, use_precond=pre, n_inner=k, sloppy_prec=F32, delta=0.1)
+        sol[name] = dict(seconds=s["seconds"], outer_iters=s["iters"], reliable_updates=s["reliable_updates"],
+                         inner_applies=s["inner_applies"], true_res=s["true_res"], rc=s["rc"])
+    ex["solve_tol1e-10_fp32outer_fp16inner"] = sol
+    del x
+    g.close()
+    torch.cuda.empty_cache()
+    g2 = Mspcg(dims, Ls, cfg["b"], cfg["c"], cfg["M5"], cfg["mf"], block)
+    g2.configure(F16, F64, 18)
+    g2.load_gauge(U, -1)
+    ex["DdagD_fp16"] = time_op(g2, F16, 2)
+    ex["Mpre_k%d_fp64" % k] = time_pre(g2, F64, 8, 8)
+    g2.close()
+    return ex
+
+
+def oracle_sample(cfg, U, src, geo):
+    """The bounded CPU sample: the oracle's M^-1 on ONE Dirichlet block (k inner iterations) + one full-lattice
+    D^dag D, fp64, plain C with OpenMP over sites.  Returns (callable running one sample, flops of the sample, ora)."""
+    from oracle.cbind import OracleC
+    dims, Ls, block, k = cfg["dims"], cfg["Ls"], cfg["block"], cfg["n_inner"]
+    ora = OracleC(dims, Ls, cfg["b"], cfg["c"], cfg["M5"], cfg["mf"], block)
+    ora.load_gauge(U, -1)
+    fl_pre, _ = precond_work(geo, Ls, k, 8, 8, 18)
+    flops = fl_pre / geo["nblk"] + flops_normal(stage_sites(geo, True), Ls)
+
+    def run():
+        ora.apply_precond(src, k, only_block=0)
+        ora.apply_MdagM(src)
+    return run, flops, ora
+
+
+def cpu_baseline(cfg, U, src, geo):
+    run, flops, ora = oracle_sample(cfg, U, src, geo)
+    t0 = time.time()
+    run()
+    dt = time.time() - t0
+    return dict(value=flops / dt / 1e9, unit=UNIT, cores=ora.threads, kind="oracle", seconds=dt,
+                sample="oracle M_pre on 1 of %d blocks (k=%d) + 1 full-lattice DdagD, fp64, same lattice" % (geo["nblk"], cfg["n_inner"]))
+
+
+def host_geometry(cfg):
+    from paper_2104_05615_b200 import Mspcg
+    m = Mspcg(cfg["dims"], cfg["Ls"], cfg["b"], cfg["c"], cfg["M5"], cfg["mf"], cfg["block"])
+    geo = m.geometry()
+    m.close()
+    return geo
+
+
+def run_reference(args):
+    """The reference arm of this tier is the CPU oracle, as it stands, on the box's host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    cfg = synth.CONFIGS[args.workload]
+    U, src = make_inputs(cfg)
+    geo = host_geometry(cfg)
+    run, flops, ora = oracle_sample(cfg, U, src, geo)
+    for _ in range(args.warmup):
+        run()
+    t0 = time.time()
+    for _ in range(args.steps):
+        run()
+    dt = (time.time() - t0) / args.steps
+    val = flops / dt / 1e9
+    dims, Ls, block, k = cfg["dims"], cfg["Ls"], cfg["block"], cfg["n_inner"]
+    sample = "oracle M_pre on 1 of %d blocks (k=%d) + 1 full-lattice DdagD per step, fp64" % (geo["nblk"], k)
+    print(json.dumps(dict(
+        metric=METRIC, value=val, unit=UNIT, n_gpus=int(os.environ.get("WORLD_SIZE", "1")), steps=args.steps, warmup=args.warmup,
+        ms_per_step=dt * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+        impl="reference",
+        config=dict(workload=f"{args.workload}: {dims[0]}x{dims[1]}x{dims[2]}x{dims[3]} Ls={Ls} blocks {block} (bounded sample)",
+                    parallelism="host cores"),
+        gpu_launches=0,
+        cpu_baseline=dict(value=val, unit=UNIT, cores=ora.threads, kind="oracle", sample=sample),
+        e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C2", choices=sorted(synth.CONFIGS))
+    ap.add_argument("--no-extras", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
