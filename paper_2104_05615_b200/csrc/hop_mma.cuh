@@ -1,0 +1,382 @@
+// hop_mma.cuh -- the fused hop kernel for fp16 storage (the preconditioner's hot path): one WARP
+// owns one 4D site and its whole fifth-dimension column; the SU(3) x spinor products and the Ls x Ls fifth-dimension
+// contractions both run on the tensor cores with fp16 operands (exactly the stored values) and fp32 accumulation,
+// so the only CUDA-core arithmetic left is the gamma-matrix recombination (64 FMAs per site column) and conversions.
+//
+// fp16 vector layout in HBM (private NATIVE layout of the __half storage type, see ST<__half> in kernels.cuh):
+//     v[site][s][colour t (3)][sp (2)][hi (2)][re,im]          spin = 2*hi + sp   (hi = 0: P+ rows, hi = 1: P- rows)
+// i.e. 48 contiguous bytes per (site, s), three 16-byte chunks, one per colour.  Lane (g = lane/4, t = lane%4) of the
+// warp loads the chunk of colour t for s = g and s = 8 + g: two 128-bit loads that ARE the A fragments of
+// mma.m16n8k16 for the four M-tiles (seg = s/8, sp) with rows (hi, g) and K = (colour, re/im) (lanes t = 3 pad K with
+// zeros).  The B fragment is the link as a real 6x6 (padded 8x8) matrix, built from one 32-bit load per lane.
+//
+//   hop (eq. 8):   sum_d (1 + sigma_d gamma_mu) W_d psi_d  =  S + sg * sum_mu gamma_mu Delta_mu,
+//       S = sum_d W_d psi_d (accumulated in one fragment set over all eight directions),
+//       Delta_mu = W_b psi_b - W_f psi_f (one k=16 MMA per M-tile: forward and backward neighbour side by side in K,
+//       the forward half of B negated), and gamma_mu only permutes (sp, hi) and swaps re/im inside a lane.
+//   5D matrices: out[s][n] = sum_s' M_hi[s][s'] X[s'][n]; the accumulator fragment is
+//       converted to fp16 (the paper's HMMA operands), transposed across the warp with movmatrix into a
+//       B fragment, and multiplied by the constant A fragment of M (host-built, one uint4 per lane and chirality).
+#pragma once
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace mspcg {
+
+template <int LS> struct MmaCfg {
+  enum { NSEG = LS > 8 ? 2 : 1, N0 = LS > 8 ? 8 : LS, N1 = LS > 8 ? LS - 8 : 0, NMT = 2 * NSEG, NW = 4 };
+};
+
+__device__ __forceinline__ void mma16816(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
+               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+               : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ uint32_t movmatrix_trans(uint32_t x) {
+  uint32_t y;
+  asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;\n" : "=r"(y) : "r"(x));
+  return y;
+}
+__device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
+  __half2 h = __floats2half2_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&h);
+}
+__device__ __forceinline__ float2 unpack_h2(uint32_t u) { return __half22float2(*reinterpret_cast<__half2*>(&u)); }
+
+// Fragment of the vector at `site`: f[seg] = 16-byte chunk of colour t at s = 8*seg + g (zero where the lane pads).
+template <int LS>
+__device__ __forceinline__ void load_frag(const __half* __restrict__ base, long site, int g, int t, uint4 (&f)[MmaCfg<LS>::NSEG], bool ok = true) {
+  typedef MmaCfg<LS> Cfg;
+  const uint4* p = reinterpret_cast<const uint4*>(base) + (ok ? site : 0) * (LS * 3) + g * 3 + t;
+  f[0] = (ok && t < 3 && g < Cfg::N0) ? __ldg(p) : make_uint4(0, 0, 0, 0);
+  if (Cfg::NSEG == 2) f[Cfg::NSEG - 1] = (ok && t < 3 && g < Cfg::N1) ? __ldg(p + 24) : make_uint4(0, 0, 0, 0);
+}
+template <int LS>
+__device__ __forceinline__ void store_frag(__half* __restrict__ base, long site, int g, int t, const uint4 (&f)[MmaCfg<LS>::NSEG]) {
+  typedef MmaCfg<LS> Cfg;
+  uint4* p = reinterpret_cast<uint4*>(base) + site * (LS * 3) + g * 3 + t;
+  if (t < 3 && g < Cfg::N0) p[0] = f[0];
+  if (Cfg::NSEG == 2) { if (t < 3 && g < Cfg::N1) p[24] = f[Cfg::NSEG - 1]; }
+}
+
+// Raw link word of lane (g, t): the complex half2 W[c = g/2][t] of the stored link (ng = 18: nine complex halves
+// row-major; ng = 12: rows 0 and 1 only, reading R8).  Loaded one site ahead; turned into a B fragment by link_bfrag.
+__device__ __forceinline__ uint32_t link_raw(const __half* __restrict__ lk, int ng, int g, int t, bool ok) {
+  const int c = g >> 1;
+  const bool mine = ok && t < 3 && g < 6 && (ng == 18 || c < 2);
+  return mine ? __ldg(reinterpret_cast<const uint32_t*>(lk) + c * 3 + t) : 0u;
+}
+// B fragment of one link: lane (g, t) supplies B[k = (colour t, re/im)][n = g = (row colour c = g/2, re/im = g%2)],
+// i.e. (Wr, -Wi) for the real output column and (Wi, Wr) for the imaginary one.  With ng = 12 the lanes of row 2 get
+// conj(row0 x row1) from the lanes holding rows 0 and 1 (lane t' holds a_t', lane 8 + t' holds b_t').  Executed by
+// the whole warp (shuffles).  `neg` folds the antiperiodic-boundary sign (R7), `have` = the neighbour contributes.
+__device__ __forceinline__ uint32_t link_bfrag(uint32_t raw, int ng, int g, int t, bool neg, bool have) {
+  uint32_t w = raw;
+  if (ng == 12) {
+    const int tt = t == 3 ? 0 : t;
+    const int t1 = tt == 2 ? 0 : tt + 1, t2 = tt == 0 ? 2 : tt - 1;   // (t+1)%3, (t+2)%3
+    const float2 a1 = unpack_h2(__shfl_sync(0xffffffffu, raw, t1)), b2 = unpack_h2(__shfl_sync(0xffffffffu, raw, 8 + t2));
+    const float2 a2 = unpack_h2(__shfl_sync(0xffffffffu, raw, t2)), b1 = unpack_h2(__shfl_sync(0xffffffffu, raw, 8 + t1));
+    const float re = (a1.x * b2.x - a1.y * b2.y) - (a2.x * b1.x - a2.y * b1.y);
+    const float im = (a1.x * b2.y + a1.y * b2.x) - (a2.x * b1.y + a2.y * b1.x);
+    if ((g >> 1) == 2) w = pack_h2(re, -im);
+  }
+  // w = (Wr, Wi):  even g -> (Wr, -Wi);  odd g -> (Wi, Wr)
+  w = (g & 1) ? __byte_perm(w, 0, 0x1032) : (w ^ 0x80000000u);
+  if (neg) w ^= 0x80008000u;
+  return (have && t < 3 && g < 6) ? w : 0u;
+}
+
+// S += sg * gamma_mu Delta for the two M-tiles (sp = 0, 1) of one segment.  Index [sp][hi*2 + ri]; gamma matrices in
+// the chiral basis of reading R2: (g_k D)_u = -i sigma_k D_l, (g_k D)_l = +i sigma_k D_u, (g_4 D)_u = D_l, (g_4 D)_l = D_u.
+template <int MU>
+__device__ __forceinline__ void gamma_accum(float (*S)[4], const float (*D)[4], float sg) {
+  if (MU == 0) {         // u0 += -i l1, u1 += -i l0, l0 += i u1, l1 += i u0
+    S[0][0] += sg * D[1][3]; S[0][1] -= sg * D[1][2]; S[1][0] += sg * D[0][3]; S[1][1] -= sg * D[0][2];
+    S[0][2] -= sg * D[1][1]; S[0][3] += sg * D[1][0]; S[1][2] -= sg * D[0][1]; S[1][3] += sg * D[0][0];
+  } else if (MU == 1) {  // u0 -= l1, u1 += l0, l0 += u1, l1 -= u0
+    S[0][0] -= sg * D[1][2]; S[0][1] -= sg * D[1][3]; S[1][0] += sg * D[0][2]; S[1][1] += sg * D[0][3];
+    S[0][2] += sg * D[1][0]; S[0][3] += sg * D[1][1]; S[1][2] -= sg * D[0][0]; S[1][3] -= sg * D[0][1];
+  } else if (MU == 2) {  // u0 += -i l0, u1 += i l1, l0 += i u0, l1 += -i u1
+    S[0][0] += sg * D[0][3]; S[0][1] -= sg * D[0][2]; S[1][0] -= sg * D[1][3]; S[1][1] += sg * D[1][2];
+    S[0][2] -= sg * D[0][1]; S[0][3] += sg * D[0][0]; S[1][2] += sg * D[1][1]; S[1][3] -= sg * D[1][0];
+  } else {               // u += l, l += u
+    S[0][0] += sg * D[0][2]; S[0][1] += sg * D[0][3]; S[1][0] += sg * D[1][2]; S[1][1] += sg * D[1][3];
+    S[0][2] += sg * D[0][0]; S[0][3] += sg * D[0][1]; S[1][2] += sg * D[1][0]; S[1][3] += sg * D[1][1];
+  }
+}
+
+// One direction pair mu: S += W_f psi_f + W_b psi_b + sg gamma_mu (W_b psi_b - W_f psi_f).
+template <int MU, int LS>
+__device__ __forceinline__ void hop_mu(float (&S)[MmaCfg<LS>::NMT][4], const uint4 (&F)[MmaCfg<LS>::NSEG], const uint4 (&B)[MmaCfg<LS>::NSEG],
+                                       uint32_t bf, uint32_t bb, float sg) {
+  typedef MmaCfg<LS> Cfg;
+  float D[Cfg::NMT][4];
+#pragma unroll
+  for (int m = 0; m < Cfg::NMT; m++) { D[m][0] = D[m][1] = D[m][2] = D[m][3] = 0.f; }
+  const uint32_t bfn = bf ^ 0x80008000u;
+#pragma unroll
+  for (int seg = 0; seg < Cfg::NSEG; seg++) {
+    mma16816(S[2 * seg], F[seg].x, F[seg].y, B[seg].x, B[seg].y, bf, bb);
+    mma16816(D[2 * seg], F[seg].x, F[seg].y, B[seg].x, B[seg].y, bfn, bb);
+    mma16816(S[2 * seg + 1], F[seg].z, F[seg].w, B[seg].z, B[seg].w, bf, bb);
+    mma16816(D[2 * seg + 1], F[seg].z, F[seg].w, B[seg].z, B[seg].w, bfn, bb);
+    gamma_accum<MU>(&S[2 * seg], &D[2 * seg], sg);
+  }
+}
+
+// X <- M X over the fifth dimension (both chiralities): X is the accumulator fragment set [seg*2+sp][hi*2+ri];
+// mfrag[hi*32 + lane] is the A fragment of the 16x16 zero-padded matrix of chirality hi.
+template <int LS>
+__device__ __forceinline__ void dense5d_mma(float (&X)[MmaCfg<LS>::NMT][4], const uint4* __restrict__ mfrag, int lane) {
+  typedef MmaCfg<LS> Cfg;
+#pragma unroll
+  for (int hi = 0; hi < 2; hi++) {
+    const uint4 A = __ldg(mfrag + hi * 32 + lane);
+#pragma unroll
+    for (int sp = 0; sp < 2; sp++) {
+      const uint32_t b0 = movmatrix_trans(pack_h2(X[sp][2 * hi], X[sp][2 * hi + 1]));
+      uint32_t b1 = 0u;
+      if (Cfg::NSEG == 2) b1 = movmatrix_trans(pack_h2(X[Cfg::NMT - 2 + sp][2 * hi], X[Cfg::NMT - 2 + sp][2 * hi + 1]));
+      float d[4] = {0.f, 0.f, 0.f, 0.f};
+      mma16816(d, A.x, A.y, A.z, A.w, b0, b1);
+      X[sp][2 * hi] = d[0]; X[sp][2 * hi + 1] = d[1];
+      if (Cfg::NSEG == 2) { X[Cfg::NMT - 2 + sp][2 * hi] = d[2]; X[Cfg::NMT - 2 + sp][2 * hi + 1] = d[3]; }
+    }
+  }
+}
+
+template <int LS>
+__device__ __forceinline__ void frag_to_float(const uint4 (&f)[MmaCfg<LS>::NSEG], float (&X)[MmaCfg<LS>::NMT][4]) {
+#pragma unroll
+  for (int seg = 0; seg < MmaCfg<LS>::NSEG; seg++) {
+    float2 q;
+    q = unpack_h2(f[seg].x); X[2 * seg][0] = q.x; X[2 * seg][1] = q.y;
+    q = unpack_h2(f[seg].y); X[2 * seg][2] = q.x; X[2 * seg][3] = q.y;
+    q = unpack_h2(f[seg].z); X[2 * seg + 1][0] = q.x; X[2 * seg + 1][1] = q.y;
+    q = unpack_h2(f[seg].w); X[2 * seg + 1][2] = q.x; X[2 * seg + 1][3] = q.y;
+  }
+}
+template <int LS>
+__device__ __forceinline__ void float_to_frag(const float (&X)[MmaCfg<LS>::NMT][4], uint4 (&f)[MmaCfg<LS>::NSEG]) {
+#pragma unroll
+  for (int seg = 0; seg < MmaCfg<LS>::NSEG; seg++) {
+    f[seg].x = pack_h2(X[2 * seg][0], X[2 * seg][1]); f[seg].y = pack_h2(X[2 * seg][2], X[2 * seg][3]);
+    f[seg].z = pack_h2(X[2 * seg + 1][0], X[2 * seg + 1][1]); f[seg].w = pack_h2(X[2 * seg + 1][2], X[2 * seg + 1][3]);
+  }
+}
+
+// ---- per-warp TMA staging (cp.async.bulk, mbarrier) ------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+template <int LS> struct MmaSmem {
+  enum { SLOT = LS * 48, STAGE = 8 * SLOT, WARP = 2 * STAGE + 64, BLOCK = MmaCfg<LS>::NW * WARP };   // bytes
+};
+
+// The fused hop kernel, fp16 storage.  Same arguments and epilogues as k_hop (kernels.cuh); a.frag1 / a.frag2 are the
+// A fragments of the fifth-dimension matrices.  Persistent warps: grid = (gx, nblk), block = 32 * NW threads; warp w of
+// the gx*NW warps of a block row takes sites w, w + gx*NW, ...   Every warp runs its own two-stage pipeline:
+//   * the eight neighbour columns of a site (Ls*48 contiguous bytes each) are fetched by eight cp.async.bulk copies
+//     (one per lane 0..7) into the warp's shared-memory stage and signalled on the warp's mbarrier; the copies of
+//     site i+1 are issued before site i is computed, so a full site is always in flight per warp;
+//   * neighbour tables, link words, boundary-flip byte and the xpay operand are register-prefetched two sites ahead
+//     in two ping-pong register sets (no register is copied, so no step waits for a load it has just issued);
+//   * the A fragments are 128-bit shared-memory reads (conflict-free: a quarter warp reads 112 contiguous bytes).
+// Slots of absent neighbours (Dirichlet cut) keep stale finite data and meet a zero B fragment.
+template <int LS, int EPI>
+__global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArgs<__half> a) {
+  typedef MmaCfg<LS> Cfg;
+  typedef MmaSmem<LS> SM;
+  constexpr int NSEG = Cfg::NSEG, NMT = Cfg::NMT, NW = Cfg::NW;
+  extern __shared__ __align__(128) unsigned char smraw[];
+  __shared__ double red[NW];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int g = lane >> 2, t = lane & 3;
+  const int blk = blockIdx.y;
+  const int stride = gridDim.x * NW;
+  const float sg = (float)a.sg;
+  float part = 0.f;
+
+  // per-block-row base pointers (64-bit once); everything below is 32-bit offsets in units of uint4
+  const uint4* in4 = reinterpret_cast<const uint4*>(a.in) + (long)blk * a.in_stride * (LS * 3);
+  uint4* out4 = reinterpret_cast<uint4*>(a.out) + (long)blk * a.out_stride * (LS * 3);
+  uint4* out24 = EPI == EPI_K3 ? reinterpret_cast<uint4*>(a.out2) + (long)blk * a.out2_stride * (LS * 3) : nullptr;
+  const uint4* aux4 = EPI != EPI_PLAIN ? reinterpret_cast<const uint4*>(a.aux) + (long)blk * a.aux_stride * (LS * 3) : nullptr;
+  const uint4* dot4 = (EPI == EPI_XPAY && a.dot_out) ? reinterpret_cast<const uint4*>(a.dotv) + (long)blk * a.dotv_stride * (LS * 3) : nullptr;
+  const uint32_t* lk32 = reinterpret_cast<const uint32_t*>(a.links) + (long)blk * a.link_stride * (4 * a.ng);
+  const uint8_t* flp = a.flip + (long)blk * a.link_stride;
+  const int* nbr = a.nbr;
+
+  // lane constants: fragment offset inside a site column (pad lanes clamped onto valid data, they meet zeros in B)
+  const int tt = t < 3 ? t : 2;
+  const int g0 = g < Cfg::N0 ? g : Cfg::N0 - 1;
+  const int g1 = Cfg::NSEG == 2 ? (g < Cfg::N1 ? g : Cfg::N1 - 1) : 0;
+  const int fo0 = g0 * 3 + tt, fo1 = 24 + g1 * 3 + tt;             // uint4 units
+  const bool st0 = t < 3 && g < Cfg::N0, st1 = Cfg::NSEG == 2 && t < 3 && g < Cfg::N1;
+  const int lko = ((g >> 1) * 3 + tt);                              // link word of this lane
+  const bool lk_mine = t < 3 && g < 6 && (a.ng == 18 || (g >> 1) < 2);
+
+  unsigned char* wsm = smraw + warp * SM::WARP;
+  const uint32_t stage_u32 = smem_u32(wsm);
+  const uint32_t bar_u32 = stage_u32 + 2 * SM::STAGE;
+  {  // zero the stages once (absent neighbours are never copied), init the two mbarriers
+    uint4* z = reinterpret_cast<uint4*>(wsm);
+    for (int i = lane; i < 2 * SM::STAGE / 16; i += 32) z[i] = make_uint4(0, 0, 0, 0);
+    if (lane == 0) { mbar_init(bar_u32, 1); mbar_init(bar_u32 + 8, 1); }
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+    __syncwarp();
+  }
+
+  struct Meta { int nbv; uint32_t lk[8]; unsigned fl; uint4 aux[NSEG]; };
+  auto ld_meta = [&](int st, Meta& m) {
+    const bool ok = st < a.n_out;
+    m.nbv = (ok && lane < 8) ? __ldg(nbr + st * 8 + lane) : -1;
+    m.fl = ok ? (unsigned)__ldg(flp + st) : 0u;
+    const uint32_t* lk = lk32 + st * (4 * a.ng) + lko;
+#pragma unroll
+    for (int d = 0; d < 8; d++) m.lk[d] = (ok && lk_mine) ? __ldg(lk + d * (a.ng >> 1)) : 0u;
+  };
+  auto ld_aux = [&](int st, Meta& m) {
+    if (EPI != EPI_PLAIN) {
+      const bool ok = st < a.n_out && st < a.n_aux;
+      const uint4* p = aux4 + st * (LS * 3);
+      m.aux[0] = (ok && st0) ? __ldg(p + fo0) : make_uint4(0, 0, 0, 0);
+      if (NSEG == 2) m.aux[NSEG - 1] = (ok && st1) ? __ldg(p + fo1) : make_uint4(0, 0, 0, 0);
+    }
+  };
+  // issue the eight neighbour copies of the site whose table is m.nbv into stage `stg`
+  auto issue = [&](const Meta& m, int stg) {
+    const bool v = lane < 8 && m.nbv >= 0 && m.nbv < a.n_in_limit;
+    const unsigned mask = __ballot_sync(0xffffffffu, v);
+    const uint32_t bar = bar_u32 + 8 * stg;
+    if (lane == 0) mbar_expect_tx(bar, (uint32_t)__popc(mask) * SM::SLOT);
+    __syncwarp();
+    if (v) bulk_g2s(stage_u32 + stg * SM::STAGE + lane * SM::SLOT, in4 + (long)m.nbv * (LS * 3), SM::SLOT, bar);
+  };
+
+  auto step = [&](int site, int stg, uint32_t parity, Meta& cur, const Meta& nxt) {
+    const int far = site + 2 * stride;
+    uint4 dv[NSEG];
+    if (EPI == EPI_XPAY && dot4 != nullptr) {
+      const uint4* p = dot4 + site * (LS * 3);
+      dv[0] = st0 ? __ldg(p + fo0) : make_uint4(0, 0, 0, 0);
+      if (NSEG == 2) dv[NSEG - 1] = st1 ? __ldg(p + fo1) : make_uint4(0, 0, 0, 0);
+    }
+    issue(nxt, stg ^ 1);                       // site + stride (a harmless empty transaction past the end)
+    const unsigned have = __ballot_sync(0xffffffffu, cur.nbv >= 0 && cur.nbv < a.n_in_limit) & 0xffu;
+    uint32_t bfr[8];
+#pragma unroll
+    for (int d = 0; d < 8; d++) bfr[d] = link_bfrag(cur.lk[d], a.ng, g, t, (cur.fl >> d) & 1u, (have >> d) & 1u);
+    ld_meta(far, cur);
+
+    float S[NMT][4];
+#pragma unroll
+    for (int m = 0; m < NMT; m++) { S[m][0] = S[m][1] = S[m][2] = S[m][3] = 0.f; }
+    mbar_wait(bar_u32 + 8 * stg, parity);
+    const uint4* sb = reinterpret_cast<const uint4*>(wsm + stg * SM::STAGE);
+#define MSPCG_HOP_MU(MU)                                                                       \
+    if (have & (3u << (2 * MU))) {                                                             \
+      uint4 Ff[NSEG], Bb[NSEG];                                                                \
+      Ff[0] = sb[(2 * MU) * (LS * 3) + fo0]; Bb[0] = sb[(2 * MU + 1) * (LS * 3) + fo0];        \
+      if (NSEG == 2) { Ff[NSEG - 1] = sb[(2 * MU) * (LS * 3) + fo1]; Bb[NSEG - 1] = sb[(2 * MU + 1) * (LS * 3) + fo1]; } \
+      hop_mu<MU, LS>(S, Ff, Bb, bfr[2 * MU], bfr[2 * MU + 1], sg);                             \
+    }
+    MSPCG_HOP_MU(0) MSPCG_HOP_MU(1) MSPCG_HOP_MU(2) MSPCG_HOP_MU(3)
+#undef MSPCG_HOP_MU
+    __syncwarp();                              // the stage may be overwritten by the copies issued in the next step
+
+    dense5d_mma<LS>(S, a.frag1, lane);
+
+    uint4 o[NSEG];
+    uint4* po = out4 + site * (LS * 3);
+    if (EPI == EPI_PLAIN) {
+      float_to_frag<LS>(S, o);
+      if (st0) po[fo0] = o[0];
+      if (NSEG == 2) { if (st1) po[fo1] = o[NSEG - 1]; }
+    } else {
+      float V[NMT][4];
+      frag_to_float<LS>(cur.aux, V);
+      ld_aux(far, cur);
+#pragma unroll
+      for (int m = 0; m < NMT; m++) {
+#pragma unroll
+        for (int q = 0; q < 4; q++) S[m][q] = V[m][q] - S[m][q];
+      }
+      float_to_frag<LS>(S, o);
+      if (EPI == EPI_K3) {
+        if (site < a.n_out2) {
+          uint4* p2 = out24 + site * (LS * 3);
+          if (st0) p2[fo0] = o[0];
+          if (NSEG == 2) { if (st1) p2[fo1] = o[NSEG - 1]; }
+        }
+        dense5d_mma<LS>(S, a.frag2, lane);
+        float_to_frag<LS>(S, o);
+      }
+      if (st0) po[fo0] = o[0];
+      if (NSEG == 2) { if (st1) po[fo1] = o[NSEG - 1]; }
+      if (EPI == EPI_XPAY && dot4 != nullptr) {
+        float P[NMT][4];
+        frag_to_float<LS>(dv, P);
+        if (st0 || st1) {
+#pragma unroll
+          for (int m = 0; m < NMT; m++) {
+#pragma unroll
+            for (int q = 0; q < 4; q++) part += P[m][q] * S[m][q];
+          }
+        }
+      }
+    }
+  };
+
+  const int site0 = blockIdx.x * NW + warp;
+  Meta mA, mB;
+  ld_meta(site0, mA); ld_meta(site0 + stride, mB);
+  ld_aux(site0, mA); ld_aux(site0 + stride, mB);
+  issue(mA, 0);
+  uint32_t par = 0;
+  for (int site = site0; site < a.n_out; site += 2 * stride) {
+    step(site, 0, par, mA, mB);
+    if (site + stride < a.n_out) step(site + stride, 1, par, mB, mA);
+    par ^= 1u;
+  }
+  // drain: a copy set may still be in flight for a site past the end (only when its table was valid: never, the
+  // tables of sites >= n_out are -1, so the last issue carried zero bytes and completed at once)
+
+  if (EPI == EPI_XPAY) {
+    if (a.dot_out != nullptr) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+      if (lane == 0) red[warp] = (double)part;
+      __syncthreads();
+      if (threadIdx.x == 0) {
+        double tot = 0;
+#pragma unroll
+        for (int w = 0; w < NW; w++) tot += red[w];
+        atomicAdd(a.dot_out + (long)blk * a.dot_stride, tot);
+      }
+    }
+  }
+}
+
+}  // namespace mspcg

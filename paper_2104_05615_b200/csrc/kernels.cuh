@@ -42,12 +42,29 @@ __device__ __forceinline__ void packV(uint4& q, const float* v) {
 }
 
 // 24 reals of (site, s); `site` is the global site index in the array (block offset already added).
+// fp64 / fp32: site-slab layout v[site][chunk][s][16 B].  fp16: v[site][s][colour][sp][hi][re,im] with spin = 2*hi+sp
+// (48 contiguous bytes per (site, s); the fragment layout of hop_mma.cuh), chunk c = colour.
+template <typename T> struct Lay {   // V-index of chunk c of (site, s) and position of real k inside the 24
+  static __device__ __forceinline__ long idx(long site, int s, int LS, int c) { return (site * ST<T>::NCH + c) * LS + s; }
+  static __device__ __forceinline__ int k(int c, int e) { return c * ST<T>::PER + e; }
+};
+template <> struct Lay<__half> {
+  static __device__ __forceinline__ long idx(long site, int s, int LS, int c) { return (site * LS + s) * 3 + c; }
+  // element e of the colour-c chunk: sp = e>>2, hi = (e>>1)&1, ri = e&1  ->  k = ((2*hi+sp)*3 + c)*2 + ri
+  static __device__ __forceinline__ int k(int c, int e) { return ((2 * ((e >> 1) & 1) + (e >> 2)) * 3 + c) * 2 + (e & 1); }
+};
 template <typename T>
 __device__ __forceinline__ void load24(const T* __restrict__ base, long site, int s, int LS, typename ST<T>::C* v) {
   typedef typename ST<T>::V V;
-  const V* p = reinterpret_cast<const V*>(base) + (site * ST<T>::NCH) * LS + s;
+  const V* p = reinterpret_cast<const V*>(base);
 #pragma unroll
-  for (int c = 0; c < ST<T>::NCH; c++) { V q = __ldg(p + c * LS); unpackV(q, v + c * ST<T>::PER); }
+  for (int c = 0; c < ST<T>::NCH; c++) {
+    V q = __ldg(p + Lay<T>::idx(site, s, LS, c));
+    typename ST<T>::C w[ST<T>::PER];
+    unpackV(q, w);
+#pragma unroll
+    for (int e = 0; e < ST<T>::PER; e++) v[Lay<T>::k(c, e)] = w[e];
+  }
 }
 template <typename T>
 __device__ __forceinline__ void load24_pred(const T* __restrict__ base, long site, int s, int LS, bool ok, typename ST<T>::C* v) {
@@ -60,9 +77,15 @@ __device__ __forceinline__ void load24_pred(const T* __restrict__ base, long sit
 template <typename T>
 __device__ __forceinline__ void store24(T* __restrict__ base, long site, int s, int LS, const typename ST<T>::C* v) {
   typedef typename ST<T>::V V;
-  V* p = reinterpret_cast<V*>(base) + (site * ST<T>::NCH) * LS + s;
+  V* p = reinterpret_cast<V*>(base);
 #pragma unroll
-  for (int c = 0; c < ST<T>::NCH; c++) { V q; packV(q, v + c * ST<T>::PER); p[c * LS] = q; }
+  for (int c = 0; c < ST<T>::NCH; c++) {
+    typename ST<T>::C w[ST<T>::PER];
+#pragma unroll
+    for (int e = 0; e < ST<T>::PER; e++) w[e] = v[Lay<T>::k(c, e)];
+    V q; packV(q, w);
+    p[Lay<T>::idx(site, s, LS, c)] = q;
+  }
 }
 
 __device__ __forceinline__ double toD(double x) { return x; }
@@ -138,6 +161,7 @@ template <typename T> struct HopArgs {
   const T* links; const uint8_t* flip; long link_stride;  // [blk][link_stride][8][ng], [blk][link_stride]
   int n_out, ng;
   const C* mat1; const C* mat2;                    // device [2][LS][LS], transposed per chirality
+  const uint4* frag1; const uint4* frag2;          // fp16 path: the same matrices as mma A fragments [2][32] (hop_mma.cuh)
   C sg;                                            // +1: D^w, -1: D^w^dag
 };
 
@@ -270,6 +294,10 @@ __global__ void __launch_bounds__(Tile<LS>::NT, (sizeof(typename ST<T>::C) == 8 
     if (tid == 0) atomicAdd(a.dot_out + (long)blk * a.dot_stride, tot);
   }
 }
+
+}  // namespace mspcg
+#include "hop_mma.cuh"
+namespace mspcg {
 
 // ------------------------------------------------------------------ K1: Mphi (bidiagonal in s), fused with p-updates
 // mode 0: t = Mphi in                                      (last item of eq. 16)

@@ -15,6 +15,7 @@
 
 #include "../../include/mspcg.h"
 #include "geometry.hpp"
+#include <cuda_fp16.h>
 #include "kernels.cuh"
 
 using namespace mspcg;
@@ -38,6 +39,8 @@ struct GeomDev { int *nbrE = nullptr, *nbrO = nullptr; short *cE = nullptr, *cO 
 
 // One set of fifth-dimension matrices (device, transposed per chirality: m[ch][s'][s]) in one compute type.
 template <typename C> struct MatSet { C *K2 = nullptr, *K3a = nullptr, *K3b = nullptr, *K4 = nullptr, *K5 = nullptr; };
+// The same matrices as fp16 mma.m16n8k16 A fragments [chirality 2][lane 32] (hop_mma.cuh).
+struct MatFrag { uint4 *K2 = nullptr, *K3a = nullptr, *K3b = nullptr, *K4 = nullptr, *K5 = nullptr; };
 struct HostMats { std::vector<double> K2, K3a, K3b, K4, K5; Mat A, F, Ainv; double diag, off; };
 
 // Everything one precision needs to apply D^dag D on one geometry.
@@ -58,6 +61,7 @@ struct mspcg_ctx {
   std::vector<double> T_host;
   std::string err;
   long launches = 0;
+  int num_sms = 148;
   // optional per-launch CUDA-event timing (mspcg_timing): class = geometry*5 + kind
   bool timing = false; int cur_geom = 0;
   std::vector<cudaEvent_t> ev_pool; std::vector<int> ev_cls; size_t ev_used = 0;
@@ -68,7 +72,7 @@ struct mspcg_ctx {
   // device
   GeomDev gfull, gblk;
   int* e_int_to_cb = nullptr;
-  MatSet<double> md, md_hat; MatSet<float> mf32, mf32_hat;
+  MatSet<double> md, md_hat; MatSet<float> mf32, mf32_hat; MatFrag mfr, mfr_hat;
   OpBuf full64, fullS, blkI;     // full lattice fp64 / sloppy; block geometry in the inner precision
   void *in_r = nullptr, *in_p = nullptr, *in_q = nullptr, *in_x = nullptr;   // inner CG vectors [V5h]
   double *rho = nullptr, *pq = nullptr; float* scale = nullptr; double* sc = nullptr;  // device scalars
@@ -124,6 +128,9 @@ template <typename C> void carve_mats(Arena& a, MatSet<C>& m, int Ls) {
   size_t n = (size_t)2 * Ls * Ls;
   m.K2 = a.take<C>(n); m.K3a = a.take<C>(n); m.K3b = a.take<C>(n); m.K4 = a.take<C>(n); m.K5 = a.take<C>(n);
 }
+void carve_frags(Arena& a, MatFrag& m) {
+  m.K2 = a.take<uint4>(64); m.K3a = a.take<uint4>(64); m.K3b = a.take<uint4>(64); m.K4 = a.take<uint4>(64); m.K5 = a.take<uint4>(64);
+}
 void carve_op(Arena& a, OpBuf& o, const Geometry& g, int prec, int ng, int Ls) {
   o.prec = prec; o.ng = ng; o.have = true;
   size_t nblk = g.nblk;
@@ -137,8 +144,8 @@ void carve(mspcg_ctx* c, Arena& a) {
   const Lattice& L = c->lat;
   carve_geom(a, c->gfull, L.full); carve_geom(a, c->gblk, L.blk);
   c->e_int_to_cb = a.take<int>(L.e_int_to_cb.size());
-  carve_mats(a, c->md, c->Ls); carve_mats(a, c->mf32, c->Ls);
-  if (c->Ls_hat) { carve_mats(a, c->md_hat, c->Ls_hat); carve_mats(a, c->mf32_hat, c->Ls_hat); }
+  carve_mats(a, c->md, c->Ls); carve_mats(a, c->mf32, c->Ls); carve_frags(a, c->mfr);
+  if (c->Ls_hat) { carve_mats(a, c->md_hat, c->Ls_hat); carve_mats(a, c->mf32_hat, c->Ls_hat); carve_frags(a, c->mfr_hat); }
   c->rho = a.take<double>((size_t)(KMAX + 1) * L.nblk); c->pq = a.take<double>((size_t)KMAX * L.nblk);
   c->scale = a.take<float>(L.nblk); c->sc = a.take<double>(16);
   carve_op(a, c->full64, L.full, MSPCG_F64, 18, c->Ls);
@@ -185,12 +192,23 @@ template <typename T, int LS, int EPI> size_t hop_smem() {
 }
 template <typename T, int LS, int EPI>
 cudaError_t launch_hop(mspcg_ctx* c, const HopArgs<T>& a, int nblk, cudaStream_t st) {
-  static bool attr = false;
-  const size_t sm = hop_smem<T, LS, EPI>();
-  if (!attr) { cudaFuncSetAttribute(k_hop<T, LS, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); attr = true; }
-  dim3 block(LS, Tile<LS>::NS), grid((a.n_out + Tile<LS>::NS - 1) / Tile<LS>::NS, nblk);
-  { TimedLaunch tl(c, EPI == EPI_PLAIN ? KIND_HOP_PLAIN : (EPI == EPI_K3 ? KIND_HOP_K3 : KIND_HOP_XPAY), st);
-    k_hop<T, LS, EPI><<<grid, block, sm, st>>>(a); }
+  const int kind = EPI == EPI_PLAIN ? KIND_HOP_PLAIN : (EPI == EPI_K3 ? KIND_HOP_K3 : KIND_HOP_XPAY);
+  if constexpr (std::is_same<T, __half>::value) {   // fp16 storage: warp-per-site tensor-core kernel (hop_mma.cuh)
+    constexpr int NW = MmaCfg<LS>::NW;
+    static bool attr = false;
+    const size_t sm = MmaSmem<LS>::BLOCK;
+    if (!attr) { cudaFuncSetAttribute(k_hop_mma<LS, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); attr = true; }
+    int gx = (a.n_out + NW - 1) / NW, cap = (4 * c->num_sms) / nblk;   // persistent warps: one wave of <= 4 thread blocks per SM
+    if (gx > cap) gx = cap;
+    dim3 block(32 * NW), grid(gx < 1 ? 1 : gx, nblk);
+    { TimedLaunch tl(c, kind, st); k_hop_mma<LS, EPI><<<grid, block, sm, st>>>(a); }
+  } else {
+    static bool attr = false;
+    const size_t sm = hop_smem<T, LS, EPI>();
+    if (!attr) { cudaFuncSetAttribute(k_hop<T, LS, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); attr = true; }
+    dim3 block(LS, Tile<LS>::NS), grid((a.n_out + Tile<LS>::NS - 1) / Tile<LS>::NS, nblk);
+    { TimedLaunch tl(c, kind, st); k_hop<T, LS, EPI><<<grid, block, sm, st>>>(a); }
+  }
   c->launches++;
   return cudaPeekAtLastError();
 }
@@ -242,6 +260,7 @@ template <typename T, int LS>
 cudaError_t apply_normal(mspcg_ctx* c, const OpView<T>& v, MphiArgs<T> mp, const T* p, T* q, double* dot_out, cudaStream_t st) {
   typedef typename ST<T>::C C;
   const MatSet<C>& m = MatPick<C>::get(c, v.hat);
+  const MatFrag& mf = v.hat ? c->mfr_hat : c->mfr;
   const HostMats& hm = v.hat ? c->hm_hat : c->hm;
   cudaError_t e;
   mp.t = v.t1; mp.n_sites = v.nE0; mp.diag = (C)hm.diag; mp.off = (C)hm.off; mp.mf = (C)c->mf;
@@ -251,22 +270,22 @@ cudaError_t apply_normal(mspcg_ctx* c, const OpView<T>& v, MphiArgs<T> mp, const
   a.ng = v.ng;
   // K2
   a.in = v.t1; a.in_stride = v.nE0; a.n_in_limit = v.nE0; a.out = v.tO; a.out_stride = v.nO; a.n_out = v.nO;
-  a.nbr = v.nbrO; a.links = v.linksO; a.flip = v.flipO; a.link_stride = v.nO; a.mat1 = m.K2; a.sg = (C)1;
+  a.nbr = v.nbrO; a.links = v.linksO; a.flip = v.flipO; a.link_stride = v.nO; a.mat1 = m.K2; a.frag1 = mf.K2; a.sg = (C)1;
   if ((e = launch_hop<T, LS, EPI_PLAIN>(c, a, v.nblk, st)) != cudaSuccess) return e;
   // K3
   a.in = v.tO; a.in_stride = v.nO; a.n_in_limit = v.nO; a.out = v.w; a.out_stride = v.nE; a.n_out = v.nE;
   a.out2 = v.y; a.out2_stride = v.nE0; a.n_out2 = v.nE0; a.aux = p; a.aux_stride = v.nE0; a.n_aux = v.nE0;
-  a.nbr = v.nbrE; a.links = v.linksE; a.flip = v.flipE; a.link_stride = v.nE; a.mat1 = m.K3a; a.mat2 = m.K3b;
+  a.nbr = v.nbrE; a.links = v.linksE; a.flip = v.flipE; a.link_stride = v.nE; a.mat1 = m.K3a; a.mat2 = m.K3b; a.frag1 = mf.K3a; a.frag2 = mf.K3b;
   if ((e = launch_hop<T, LS, EPI_K3>(c, a, v.nblk, st)) != cudaSuccess) return e;
   // K4
   a.in = v.w; a.in_stride = v.nE; a.n_in_limit = v.nE; a.out = v.tO; a.out_stride = v.nO; a.n_out = v.nO;
   a.out2 = nullptr; a.aux = nullptr; a.n_aux = 0; a.nbr = v.nbrO; a.links = v.linksO; a.flip = v.flipO; a.link_stride = v.nO;
-  a.mat1 = m.K4; a.mat2 = nullptr; a.sg = (C)-1;
+  a.mat1 = m.K4; a.mat2 = nullptr; a.frag1 = mf.K4; a.frag2 = nullptr; a.sg = (C)-1;
   if ((e = launch_hop<T, LS, EPI_PLAIN>(c, a, v.nblk, st)) != cudaSuccess) return e;
   // K5
   a.in = v.tO; a.in_stride = v.nO; a.n_in_limit = v.nO; a.out = q; a.out_stride = v.nE0; a.n_out = v.nE0;
   a.aux = v.y; a.aux_stride = v.nE0; a.n_aux = v.nE0; a.dotv = p; a.dotv_stride = v.nE0; a.dot_out = dot_out; a.dot_stride = 1;
-  a.nbr = v.nbrE; a.links = v.linksE; a.flip = v.flipE; a.link_stride = v.nE; a.mat1 = m.K5;
+  a.nbr = v.nbrE; a.links = v.linksE; a.flip = v.flipE; a.link_stride = v.nE; a.mat1 = m.K5; a.frag1 = mf.K5;
   return launch_hop<T, LS, EPI_XPAY>(c, a, v.nblk, st);
 }
 
@@ -392,6 +411,31 @@ template <typename C> cudaError_t upload_mats(const MatSet<C>& m, const HostMats
     cudaError_t e = cudaMemcpyAsync(dst[i], tmp.data(), tmp.size() * sizeof(C), cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return e;
     cudaStreamSynchronize(st);  // tmp goes out of scope
+  }
+  return cudaSuccess;
+}
+// fp16 A fragments of mma.m16n8k16 (row-major 16x16, zero padded) of the five matrices; src is the transposed-per-
+// chirality array of build_host_mats: M_ch[s][s'] = src[(ch*n + s')*n + s].
+cudaError_t upload_frags(const MatFrag& m, const HostMats& h, int n, cudaStream_t st) {
+  const std::vector<double>* src[5] = {&h.K2, &h.K3a, &h.K3b, &h.K4, &h.K5};
+  uint4* dst[5] = {m.K2, m.K3a, m.K3b, m.K4, m.K5};
+  for (int i = 0; i < 5; i++) {
+    std::vector<uint32_t> tmp(2 * 32 * 4);
+    auto M = [&](int ch, int s, int sp) -> float { return (s < n && sp < n) ? (float)(*src[i])[((size_t)ch * n + sp) * n + s] : 0.f; };
+    auto h2 = [&](float lo, float hi) -> uint32_t {
+      __half a = __float2half_rn(lo), b = __float2half_rn(hi); unsigned short ua, ub;
+      memcpy(&ua, &a, 2); memcpy(&ub, &b, 2); return (uint32_t)ua | ((uint32_t)ub << 16);
+    };
+    for (int ch = 0; ch < 2; ch++)
+      for (int lane = 0; lane < 32; lane++) {
+        const int g = lane >> 2, t = lane & 3;
+        uint32_t* q = &tmp[((size_t)ch * 32 + lane) * 4];
+        q[0] = h2(M(ch, g, 2 * t), M(ch, g, 2 * t + 1));         q[1] = h2(M(ch, g + 8, 2 * t), M(ch, g + 8, 2 * t + 1));
+        q[2] = h2(M(ch, g, 2 * t + 8), M(ch, g, 2 * t + 9));     q[3] = h2(M(ch, g + 8, 2 * t + 8), M(ch, g + 8, 2 * t + 9));
+      }
+    cudaError_t e = cudaMemcpyAsync(dst[i], tmp.data(), tmp.size() * 4, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return e;
+    cudaStreamSynchronize(st);
   }
   return cudaSuccess;
 }
@@ -626,7 +670,10 @@ int mspcg_set_workspace(mspcg_ctx* ctx, void* workspace_dev, size_t bytes, void*
   CUDA_OK(ctx, up(ctx->e_int_to_cb, L.e_int_to_cb, st));
   CUDA_OK(ctx, cudaStreamSynchronize(st));
   CUDA_OK(ctx, upload_mats<double>(ctx->md, ctx->hm, st)); CUDA_OK(ctx, upload_mats<float>(ctx->mf32, ctx->hm, st));
+  CUDA_OK(ctx, upload_frags(ctx->mfr, ctx->hm, ctx->Ls, st));
   if (!ctx->sc_host) CUDA_OK(ctx, cudaMallocHost(&ctx->sc_host, sizeof(double) * 16));
+  { int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0) ctx->num_sms = n; }
   ctx->have_ws = true;
   return MSPCG_OK;
 }
