@@ -60,32 +60,25 @@ __device__ __forceinline__ void store_frag(__half* __restrict__ base, long site,
   if (Cfg::NSEG == 2) { if (t < 3 && g < Cfg::N1) p[24] = f[Cfg::NSEG - 1]; }
 }
 
-// Raw link word of lane (g, t): the complex half2 W[c = g/2][t] of the stored link (ng = 18: nine complex halves
-// row-major; ng = 12: rows 0 and 1 only, reading R8).  Loaded one site ahead; turned into a B fragment by link_bfrag.
-__device__ __forceinline__ uint32_t link_raw(const __half* __restrict__ lk, int ng, int g, int t, bool ok) {
-  const int c = g >> 1;
-  const bool mine = ok && t < 3 && g < 6 && (ng == 18 || c < 2);
-  return mine ? __ldg(reinterpret_cast<const uint32_t*>(lk) + c * 3 + t) : 0u;
-}
-// B fragment of one link: lane (g, t) supplies B[k = (colour t, re/im)][n = g = (row colour c = g/2, re/im = g%2)],
-// i.e. (Wr, -Wi) for the real output column and (Wi, Wr) for the imaginary one.  With ng = 12 the lanes of row 2 get
-// conj(row0 x row1) from the lanes holding rows 0 and 1 (lane t' holds a_t', lane 8 + t' holds b_t').  Executed by
-// the whole warp (shuffles).  `neg` folds the antiperiodic-boundary sign (R7), `have` = the neighbour contributes.
-__device__ __forceinline__ uint32_t link_bfrag(uint32_t raw, int ng, int g, int t, bool neg, bool have) {
+// B fragment of one link from its raw word.  Raw word of lane (g, t): the complex half2 W[c = g/2][t] of the stored
+// link (NG = 18: nine complex halves row-major; NG = 12: rows 0 and 1 only, reading R8), zero on pad lanes.
+// Lane (g, t) supplies B[k = (colour t, re/im)][n = g = (row colour c, re/im = g%2)]: (Wr, -Wi) for the real output
+// column, (Wi, Wr) for the imaginary one -- one byte permute with the per-lane selector `sel` (0x7610 / 0x1032).
+// With NG = 12 the lanes of row 2 get conj(row0 x row1) from the lanes holding rows 0 and 1 (lane t' holds a_t',
+// lane 8 + t' holds b_t'); executed by the whole warp (shuffles).
+template <int NG>
+__device__ __forceinline__ uint32_t link_bfrag(uint32_t raw, int g, int t, uint32_t sel) {
   uint32_t w = raw;
-  if (ng == 12) {
+  if (NG == 12) {
     const int tt = t == 3 ? 0 : t;
     const int t1 = tt == 2 ? 0 : tt + 1, t2 = tt == 0 ? 2 : tt - 1;   // (t+1)%3, (t+2)%3
     const float2 a1 = unpack_h2(__shfl_sync(0xffffffffu, raw, t1)), b2 = unpack_h2(__shfl_sync(0xffffffffu, raw, 8 + t2));
     const float2 a2 = unpack_h2(__shfl_sync(0xffffffffu, raw, t2)), b1 = unpack_h2(__shfl_sync(0xffffffffu, raw, 8 + t1));
     const float re = (a1.x * b2.x - a1.y * b2.y) - (a2.x * b1.x - a2.y * b1.y);
     const float im = (a1.x * b2.y + a1.y * b2.x) - (a2.x * b1.y + a2.y * b1.x);
-    if ((g >> 1) == 2) w = pack_h2(re, -im);
+    if ((g >> 1) == 2 && t < 3) w = pack_h2(re, -im);
   }
-  // w = (Wr, Wi):  even g -> (Wr, -Wi);  odd g -> (Wi, Wr)
-  w = (g & 1) ? __byte_perm(w, 0, 0x1032) : (w ^ 0x80000000u);
-  if (neg) w ^= 0x80008000u;
-  return (have && t < 3 && g < 6) ? w : 0u;
+  return __byte_perm(w, w ^ 0x80000000u, sel);   // pad lanes: (+0, -0), harmless
 }
 
 // S += sg * gamma_mu Delta for the two M-tiles (sp = 0, 1) of one segment.  Index [sp][hi*2 + ri]; gamma matrices in
@@ -108,8 +101,10 @@ __device__ __forceinline__ void gamma_accum(float (*S)[4], const float (*D)[4], 
 }
 
 // One direction pair mu: S += W_f psi_f + W_b psi_b + sg gamma_mu (W_b psi_b - W_f psi_f).
+// F[2*seg + sp] / B[...] = (hi = 0, hi = 1) half2 pairs of the forward / backward neighbour: the A operand of M-tile
+// (seg, sp) is {F.x, F.y, B.x, B.y} (rows (hi, g), K = forward colours | backward colours).
 template <int MU, int LS>
-__device__ __forceinline__ void hop_mu(float (&S)[MmaCfg<LS>::NMT][4], const uint4 (&F)[MmaCfg<LS>::NSEG], const uint4 (&B)[MmaCfg<LS>::NSEG],
+__device__ __forceinline__ void hop_mu(float (&S)[MmaCfg<LS>::NMT][4], const uint2 (&F)[MmaCfg<LS>::NMT], const uint2 (&B)[MmaCfg<LS>::NMT],
                                        uint32_t bf, uint32_t bb, float sg) {
   typedef MmaCfg<LS> Cfg;
   float D[Cfg::NMT][4];
@@ -117,13 +112,12 @@ __device__ __forceinline__ void hop_mu(float (&S)[MmaCfg<LS>::NMT][4], const uin
   for (int m = 0; m < Cfg::NMT; m++) { D[m][0] = D[m][1] = D[m][2] = D[m][3] = 0.f; }
   const uint32_t bfn = bf ^ 0x80008000u;
 #pragma unroll
-  for (int seg = 0; seg < Cfg::NSEG; seg++) {
-    mma16816(S[2 * seg], F[seg].x, F[seg].y, B[seg].x, B[seg].y, bf, bb);
-    mma16816(D[2 * seg], F[seg].x, F[seg].y, B[seg].x, B[seg].y, bfn, bb);
-    mma16816(S[2 * seg + 1], F[seg].z, F[seg].w, B[seg].z, B[seg].w, bf, bb);
-    mma16816(D[2 * seg + 1], F[seg].z, F[seg].w, B[seg].z, B[seg].w, bfn, bb);
-    gamma_accum<MU>(&S[2 * seg], &D[2 * seg], sg);
+  for (int m = 0; m < Cfg::NMT; m++) {
+    mma16816(S[m], F[m].x, F[m].y, B[m].x, B[m].y, bf, bb);
+    mma16816(D[m], F[m].x, F[m].y, B[m].x, B[m].y, bfn, bb);
   }
+#pragma unroll
+  for (int seg = 0; seg < Cfg::NSEG; seg++) gamma_accum<MU>(&S[2 * seg], &D[2 * seg], sg);
 }
 
 // X <- M X over the fifth dimension (both chiralities): X is the accumulator fragment set [seg*2+sp][hi*2+ri];
@@ -203,7 +197,7 @@ template <int LS> struct MmaSmem {
 //     in two ping-pong register sets (no register is copied, so no step waits for a load it has just issued);
 //   * the A fragments are 128-bit shared-memory reads (conflict-free: a quarter warp reads 112 contiguous bytes).
 // Slots of absent neighbours (Dirichlet cut) keep stale finite data and meet a zero B fragment.
-template <int LS, int EPI>
+template <int LS, int EPI, int NG>
 __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArgs<__half> a) {
   typedef MmaCfg<LS> Cfg;
   typedef MmaSmem<LS> SM;
@@ -223,7 +217,7 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
   uint4* out24 = EPI == EPI_K3 ? reinterpret_cast<uint4*>(a.out2) + (long)blk * a.out2_stride * (LS * 3) : nullptr;
   const uint4* aux4 = EPI != EPI_PLAIN ? reinterpret_cast<const uint4*>(a.aux) + (long)blk * a.aux_stride * (LS * 3) : nullptr;
   const uint4* dot4 = (EPI == EPI_XPAY && a.dot_out) ? reinterpret_cast<const uint4*>(a.dotv) + (long)blk * a.dotv_stride * (LS * 3) : nullptr;
-  const uint32_t* lk32 = reinterpret_cast<const uint32_t*>(a.links) + (long)blk * a.link_stride * (4 * a.ng);
+  const uint32_t* lk32 = reinterpret_cast<const uint32_t*>(a.links) + (long)blk * a.link_stride * (4 * NG);
   const uint8_t* flp = a.flip + (long)blk * a.link_stride;
   const int* nbr = a.nbr;
 
@@ -234,7 +228,8 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
   const int fo0 = g0 * 3 + tt, fo1 = 24 + g1 * 3 + tt;             // uint4 units
   const bool st0 = t < 3 && g < Cfg::N0, st1 = Cfg::NSEG == 2 && t < 3 && g < Cfg::N1;
   const int lko = ((g >> 1) * 3 + tt);                              // link word of this lane
-  const bool lk_mine = t < 3 && g < 6 && (a.ng == 18 || (g >> 1) < 2);
+  const bool lk_mine = t < 3 && g < 6 && (NG == 18 || (g >> 1) < 2);
+  const uint32_t bsel = (g & 1) ? 0x1032u : 0x7610u;
 
   unsigned char* wsm = smraw + warp * SM::WARP;
   const uint32_t stage_u32 = smem_u32(wsm);
@@ -253,9 +248,9 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
     const bool ok = st < a.n_out;
     m.nbv = (ok && lane < 8) ? __ldg(nbr + st * 8 + lane) : -1;
     m.fl = ok ? (unsigned)__ldg(flp + st) : 0u;
-    const uint32_t* lk = lk32 + st * (4 * a.ng) + lko;
+    const uint32_t* lk = lk32 + st * (4 * NG) + lko;
 #pragma unroll
-    for (int d = 0; d < 8; d++) m.lk[d] = (ok && lk_mine) ? __ldg(lk + d * (a.ng >> 1)) : 0u;
+    for (int d = 0; d < 8; d++) m.lk[d] = (ok && lk_mine) ? __ldg(lk + d * (NG / 2)) : 0u;
   };
   auto ld_aux = [&](int st, Meta& m) {
     if (EPI != EPI_PLAIN) {
@@ -287,19 +282,24 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
     const unsigned have = __ballot_sync(0xffffffffu, cur.nbv >= 0 && cur.nbv < a.n_in_limit) & 0xffu;
     uint32_t bfr[8];
 #pragma unroll
-    for (int d = 0; d < 8; d++) bfr[d] = link_bfrag(cur.lk[d], a.ng, g, t, (cur.fl >> d) & 1u, (have >> d) & 1u);
+    for (int d = 0; d < 8; d++) {
+      uint32_t w = link_bfrag<NG>(cur.lk[d], g, t, bsel);
+      if (d >= 6) { if ((cur.fl >> d) & 1u) w ^= 0x80008000u; }   // only time links cross the antiperiodic boundary (R7)
+      bfr[d] = (have & (1u << d)) ? w : 0u;                       // absent neighbour: its slot holds stale data
+    }
     ld_meta(far, cur);
 
     float S[NMT][4];
 #pragma unroll
     for (int m = 0; m < NMT; m++) { S[m][0] = S[m][1] = S[m][2] = S[m][3] = 0.f; }
     mbar_wait(bar_u32 + 8 * stg, parity);
-    const uint4* sb = reinterpret_cast<const uint4*>(wsm + stg * SM::STAGE);
+    const uint2* sb = reinterpret_cast<const uint2*>(wsm + stg * SM::STAGE);   // 64-bit reads: (hi0, hi1) of one sp
 #define MSPCG_HOP_MU(MU)                                                                       \
     if (have & (3u << (2 * MU))) {                                                             \
-      uint4 Ff[NSEG], Bb[NSEG];                                                                \
-      Ff[0] = sb[(2 * MU) * (LS * 3) + fo0]; Bb[0] = sb[(2 * MU + 1) * (LS * 3) + fo0];        \
-      if (NSEG == 2) { Ff[NSEG - 1] = sb[(2 * MU) * (LS * 3) + fo1]; Bb[NSEG - 1] = sb[(2 * MU + 1) * (LS * 3) + fo1]; } \
+      uint2 Ff[NMT], Bb[NMT];                                                                  \
+      const uint2* pf = sb + (2 * MU) * (LS * 6); const uint2* pb = pf + LS * 6;               \
+      Ff[0] = pf[2 * fo0]; Ff[1] = pf[2 * fo0 + 1]; Bb[0] = pb[2 * fo0]; Bb[1] = pb[2 * fo0 + 1]; \
+      if (NSEG == 2) { Ff[NMT - 2] = pf[2 * fo1]; Ff[NMT - 1] = pf[2 * fo1 + 1]; Bb[NMT - 2] = pb[2 * fo1]; Bb[NMT - 1] = pb[2 * fo1 + 1]; } \
       hop_mu<MU, LS>(S, Ff, Bb, bfr[2 * MU], bfr[2 * MU + 1], sg);                             \
     }
     MSPCG_HOP_MU(0) MSPCG_HOP_MU(1) MSPCG_HOP_MU(2) MSPCG_HOP_MU(3)

@@ -197,11 +197,16 @@ cudaError_t launch_hop(mspcg_ctx* c, const HopArgs<T>& a, int nblk, cudaStream_t
     constexpr int NW = MmaCfg<LS>::NW;
     static bool attr = false;
     const size_t sm = MmaSmem<LS>::BLOCK;
-    if (!attr) { cudaFuncSetAttribute(k_hop_mma<LS, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); attr = true; }
+    if (!attr) {
+      cudaFuncSetAttribute(k_hop_mma<LS, EPI, 18>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+      cudaFuncSetAttribute(k_hop_mma<LS, EPI, 12>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+      attr = true;
+    }
     int gx = (a.n_out + NW - 1) / NW, cap = (4 * c->num_sms) / nblk;   // persistent warps: one wave of <= 4 thread blocks per SM
     if (gx > cap) gx = cap;
     dim3 block(32 * NW), grid(gx < 1 ? 1 : gx, nblk);
-    { TimedLaunch tl(c, kind, st); k_hop_mma<LS, EPI><<<grid, block, sm, st>>>(a); }
+    { TimedLaunch tl(c, kind, st);
+      if (a.ng == 12) k_hop_mma<LS, EPI, 12><<<grid, block, sm, st>>>(a); else k_hop_mma<LS, EPI, 18><<<grid, block, sm, st>>>(a); }
   } else {
     static bool attr = false;
     const size_t sm = hop_smem<T, LS, EPI>();
