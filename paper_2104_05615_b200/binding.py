@@ -153,6 +153,13 @@ class Mspcg:
         self.outer_prec, self.inner_prec = outer_prec, inner_prec
         return n.value
 
+    def set_reduced_ls(self, Ls_hat, T_abi, mu):
+        """Reduced-Ls preconditioner: T_abi = float64 [4*Ls_hat][4*Ls][re,im]; call before configure()."""
+        T = np.ascontiguousarray(T_abi, dtype=np.float64).reshape(-1)
+        assert T.size == 4 * int(Ls_hat) * 4 * self.Ls * 2
+        self._check(self.lib.mspcg_set_reduced_ls(self.h, int(Ls_hat), T.ctypes.data_as(C.POINTER(C.c_double)), float(mu)))
+        self.Ls_hat = int(Ls_hat)
+
     # ---- device set-up -----------------------------------------------------------------------------------------
     def _stream(self):
         return C.c_void_p(_torch().cuda.current_stream().cuda_stream)

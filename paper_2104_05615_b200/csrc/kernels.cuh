@@ -491,6 +491,82 @@ __global__ void k_inner_update(const T* __restrict__ p, const T* __restrict__ q,
   }
 }
 
+// ------------------------------------------------------------------ reduced-Ls transfer (generic path)
+// eq. 21: [T v]_{a,m} = sum_{s,n} T[a m, s n] v_{s,n}; T is the identity in colour and 4D site.
+// Tm = device copy of T_host[4*Lh][4*Ls][re,im] (fp64).  One thread per (site, a = s_hat):
+//   rhat = T (rin / scale[blk]) stored in T (rounded), rho0[blk] += |rhat|^2 of the stored values.
+template <typename TIO, typename T>
+__global__ void k_reduce_begin(const TIO* __restrict__ rin, T* __restrict__ rhat, long n_sites, int Ls, int Lh,
+                               const double* __restrict__ Tm, const float* scale, double* rho0) {
+  __shared__ double red[32];
+  const SiteThread t = site_thread(n_sites, Lh);
+  double part = 0;
+  if (t.live) {
+    const double f = 1.0 / blk_scale(scale, t.blk);
+    double acc[24];
+#pragma unroll
+    for (int k = 0; k < 24; k++) acc[k] = 0;
+    for (int s = 0; s < Ls; s++) {
+      typename ST<TIO>::C v[24];
+      load24<TIO>(rin, t.gsite, s, Ls, v);
+#pragma unroll
+      for (int m = 0; m < 4; m++)
+#pragma unroll
+        for (int n = 0; n < 4; n++) {
+          const double2 tc = *reinterpret_cast<const double2*>(Tm + (((long)(t.s * 4 + m)) * (4 * Ls) + s * 4 + n) * 2);
+#pragma unroll
+          for (int c = 0; c < 3; c++) {
+            const double vr = (double)v[(n * 3 + c) * 2], vi = (double)v[(n * 3 + c) * 2 + 1];
+            acc[(m * 3 + c) * 2] += tc.x * vr - tc.y * vi;
+            acc[(m * 3 + c) * 2 + 1] += tc.x * vi + tc.y * vr;
+          }
+        }
+    }
+    typename ST<T>::C o[24];
+#pragma unroll
+    for (int k = 0; k < 24; k++) {
+      o[k] = round_store((typename ST<T>::C)(acc[k] * f), (int)sizeof(T));
+      part += (double)o[k] * (double)o[k];
+    }
+    store24<T>(rhat, t.gsite, t.s, Lh, o);
+  }
+  const double tot = block_sum(part, red, threadIdx.x, blockDim.x);
+  if (threadIdx.x == 0 && tot != 0.0) atomicAdd(rho0 + t.blk, tot);
+}
+
+// z = scale[blk] * T^dag xhat + mu * rin  (eq. 20).  One thread per (site, s).
+template <typename TX, typename TIO>
+__global__ void k_reduce_end(const TX* __restrict__ xhat, const TIO* __restrict__ rin, TIO* __restrict__ z, long n_sites, int Ls,
+                             int Lh, const double* __restrict__ Tm, const float* scale, double mu) {
+  const SiteThread t = site_thread(n_sites, Ls);
+  if (!t.live) return;
+  const double f = blk_scale(scale, t.blk);
+  double acc[24];
+#pragma unroll
+  for (int k = 0; k < 24; k++) acc[k] = 0;
+  for (int a = 0; a < Lh; a++) {
+    typename ST<TX>::C v[24];
+    load24<TX>(xhat, t.gsite, a, Lh, v);
+#pragma unroll
+    for (int m = 0; m < 4; m++)
+#pragma unroll
+      for (int n = 0; n < 4; n++) {
+        const double2 tc = *reinterpret_cast<const double2*>(Tm + (((long)(a * 4 + m)) * (4 * Ls) + t.s * 4 + n) * 2);
+#pragma unroll
+        for (int c = 0; c < 3; c++) {   // conj(T) * x
+          const double vr = (double)v[(m * 3 + c) * 2], vi = (double)v[(m * 3 + c) * 2 + 1];
+          acc[(n * 3 + c) * 2] += tc.x * vr + tc.y * vi;
+          acc[(n * 3 + c) * 2 + 1] += tc.x * vi - tc.y * vr;
+        }
+      }
+  }
+  typename ST<TIO>::C r[24], o[24];
+  load24<TIO>(rin, t.gsite, t.s, Ls, r);
+#pragma unroll
+  for (int k = 0; k < 24; k++) o[k] = (typename ST<TIO>::C)(f * acc[k] + mu * (double)r[k]);
+  store24<TIO>(z, t.gsite, t.s, Ls, o);
+}
+
 // Same-precision flat kernels: one thread per 16-byte chunk.
 template <typename T> __device__ __forceinline__ void ldchunk(const T* base, long i, typename ST<T>::C* v) {
   typedef typename ST<T>::V V; V q = __ldg(reinterpret_cast<const V*>(base) + i); unpackV(q, v);

@@ -76,6 +76,7 @@ struct mspcg_ctx {
   OpBuf full64, fullS, blkI;     // full lattice fp64 / sloppy; block geometry in the inner precision
   void *in_r = nullptr, *in_p = nullptr, *in_q = nullptr, *in_x = nullptr;   // inner CG vectors [V5h]
   double *rho = nullptr, *pq = nullptr; float* scale = nullptr; double* sc = nullptr;  // device scalars
+  double* Tm = nullptr;          // device copy of the reduced-Ls transfer matrix T_host (A10)
   double* sc_host = nullptr;     // pinned
   double *v_b = nullptr, *v_xhi = nullptr, *v_rhi = nullptr, *v_t64 = nullptr;   // solver, fp64 native
   void *v_xlo = nullptr, *v_rlo = nullptr, *v_p = nullptr, *v_Ap = nullptr, *v_z = nullptr;  // solver, sloppy
@@ -148,6 +149,7 @@ void carve(mspcg_ctx* c, Arena& a) {
   if (c->Ls_hat) { carve_mats(a, c->md_hat, c->Ls_hat); carve_mats(a, c->mf32_hat, c->Ls_hat); carve_frags(a, c->mfr_hat); }
   c->rho = a.take<double>((size_t)(KMAX + 1) * L.nblk); c->pq = a.take<double>((size_t)KMAX * L.nblk);
   c->scale = a.take<float>(L.nblk); c->sc = a.take<double>(16);
+  if (c->Ls_hat) c->Tm = a.take<double>((size_t)4 * c->Ls_hat * 4 * c->Ls * 2);
   carve_op(a, c->full64, L.full, MSPCG_F64, 18, c->Ls);
   if (c->outer_prec != MSPCG_F64) carve_op(a, c->fullS, L.full, c->outer_prec, c->recon, c->Ls);
   carve_op(a, c->blkI, L.blk, c->inner_prec, c->inner_prec == MSPCG_F64 ? 18 : c->recon, c->Ls);
@@ -314,12 +316,14 @@ cudaError_t convert_any(mspcg_ctx* c, const void* a, int pa, void* b, int pb, lo
 }
 
 // ---------------------------------------------------------------------------------------- the preconditioner (A7, A8)
+// LS is the fifth-dimension extent of the inner iteration: Ls, or Ls_hat when `reduced` (then the right-hand side is
+// T r, the operator is built from the Ls_hat matrices, and z = T^dag x + mu r; eq. 19-21).
 template <typename TIO, typename T, int LS>
-cudaError_t precond_impl(mspcg_ctx* c, const TIO* r_in, TIO* z_out, int k, cudaStream_t st) {
+cudaError_t precond_impl(mspcg_ctx* c, const TIO* r_in, TIO* z_out, int k, bool reduced, cudaStream_t st) {
   typedef typename std::conditional<sizeof(T) == 8, double, float>::type TX;
   const Geometry& g = c->lat.blk;
   const int nblk = g.nblk;
-  OpView<T> v = make_view<T>(c, c->blkI, g, c->gblk, LS, false);
+  OpView<T> v = make_view<T>(c, c->blkI, g, c->gblk, LS, reduced);
   c->cur_geom = 1;
   cudaError_t e;
   if ((e = cudaMemsetAsync(c->rho, 0, sizeof(double) * (size_t)(KMAX + 1) * nblk, st)) != cudaSuccess) return e;
@@ -327,39 +331,46 @@ cudaError_t precond_impl(mspcg_ctx* c, const TIO* r_in, TIO* z_out, int k, cudaS
   const float* scale = nullptr;
   if (sizeof(T) == 2) {   // fp16 storage: rescale every block's right-hand side to max-abs 1 (R14)
     if ((e = cudaMemsetAsync(c->scale, 0, sizeof(float) * nblk, st)) != cudaSuccess) return e;
-    { TimedLaunch tl(c, KIND_BLAS, st); k_maxabs<TIO><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(r_in, g.nE0, LS, c->scale); }
+    { TimedLaunch tl(c, KIND_BLAS, st); k_maxabs<TIO><<<grid_sites(g.nE0, c->Ls, nblk), 128, 0, st>>>(r_in, g.nE0, c->Ls, c->scale); }
     c->launches++;
     scale = c->scale;
   }
   T *r = (T*)c->in_r, *p = (T*)c->in_p, *q = (T*)c->in_q; TX* x = (TX*)c->in_x;
-  { TimedLaunch tl(c, KIND_BLAS, st); k_pre_begin<TIO, T><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(r_in, r, g.nE0, LS, scale, c->rho); }
+  { TimedLaunch tl(c, KIND_BLAS, st);
+    if (reduced) k_reduce_begin<TIO, T><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(r_in, r, g.nE0, c->Ls, LS, c->Tm, scale, c->rho);
+    else k_pre_begin<TIO, T><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(r_in, r, g.nE0, LS, scale, c->rho); }
   c->launches++;
   for (int it = 0; it < k; it++) {
     MphiArgs<T> mp; memset(&mp, 0, sizeof(mp));
     mp.in = r; mp.p = p; mp.mode = 2; mp.it = it; mp.nblk = nblk; mp.rho = c->rho; mp.pq = c->pq;
     if ((e = apply_normal<T, LS>(c, v, mp, p, q, c->pq + (size_t)it * nblk, st)) != cudaSuccess) return e;
     { TimedLaunch tl(c, KIND_BLAS, st);
-      k_inner_update<T, TX, TIO><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(p, q, r, x, z_out, g.nE0, LS, it, nblk, it == k - 1,
+      k_inner_update<T, TX, TIO><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(p, q, r, x, z_out, g.nE0, LS, it, nblk, (it == k - 1 && !reduced) ? 1 : 0,
                                                                             c->rho, c->pq, scale); }
+    c->launches++;
+  }
+  if (reduced) {
+    { TimedLaunch tl(c, KIND_BLAS, st);
+      k_reduce_end<TX, TIO><<<grid_sites(g.nE0, c->Ls, nblk), 128, 0, st>>>(x, r_in, z_out, g.nE0, c->Ls, LS, c->Tm, scale, c->mu_shift); }
     c->launches++;
   }
   return cudaPeekAtLastError();
 }
 
 template <typename TIO>
-cudaError_t precond_dispatch(mspcg_ctx* c, const TIO* r, TIO* z, int k, cudaStream_t st) {
-  const int Ls = c->Ls;
+cudaError_t precond_dispatch(mspcg_ctx* c, const TIO* r, TIO* z, int k, bool reduced, cudaStream_t st) {
+  const int Ls = reduced ? c->Ls_hat : c->Ls;
   switch (c->inner_prec) {
-    case MSPCG_F64: DISPATCH_LS(Ls, return (precond_impl<TIO, double, LS>(c, r, z, k, st)));
-    case MSPCG_F32: DISPATCH_LS(Ls, return (precond_impl<TIO, float, LS>(c, r, z, k, st)));
-    default: DISPATCH_LS(Ls, return (precond_impl<TIO, __half, LS>(c, r, z, k, st)));
+    case MSPCG_F64: DISPATCH_LS(Ls, return (precond_impl<TIO, double, LS>(c, r, z, k, reduced, st)));
+    case MSPCG_F32: DISPATCH_LS(Ls, return (precond_impl<TIO, float, LS>(c, r, z, k, reduced, st)));
+    default: DISPATCH_LS(Ls, return (precond_impl<TIO, __half, LS>(c, r, z, k, reduced, st)));
   }
   return cudaErrorInvalidValue;
 }
-cudaError_t precond_any(mspcg_ctx* c, const void* r, void* z, int io_prec, int k, cudaStream_t st) {
-  if (io_prec == MSPCG_F64) return precond_dispatch<double>(c, (const double*)r, (double*)z, k, st);
-  if (io_prec == MSPCG_F32) return precond_dispatch<float>(c, (const float*)r, (float*)z, k, st);
-  return precond_dispatch<__half>(c, (const __half*)r, (__half*)z, k, st);
+cudaError_t precond_any(mspcg_ctx* c, const void* r, void* z, int io_prec, int k, bool reduced, cudaStream_t st) {
+  if (io_prec == MSPCG_F64) return precond_dispatch<double>(c, (const double*)r, (double*)z, k, reduced, st);
+  if (io_prec == MSPCG_F32) return precond_dispatch<float>(c, (const float*)r, (float*)z, k, reduced, st);
+  return precond_dispatch<__half>(c, (const __half*)r, (__half*)z, k, reduced, st);
 }
 
 // ------------------------------------------------------------------------------------------- full-lattice D^dag D
@@ -525,7 +536,7 @@ int solve_impl(mspcg_ctx* c, const double* b_abi, double* x_abi, const mspcg_sol
     maxr = rnorm;
     if (rnorm <= prm->tol * bnorm) stt->converged = 1;
     else {
-      if (prm->use_precond) { SOLVE_CUDA(precond_any(c, rlo, z, sp, prm->n_inner, st)); stt->inner_applies += (long)prm->n_inner * c->lat.nblk; }
+      if (prm->use_precond) { SOLVE_CUDA(precond_any(c, rlo, z, sp, prm->n_inner, prm->use_reduced_ls != 0, st)); stt->inner_applies += (long)prm->n_inner * c->lat.nblk; }
       SOLVE_CUDA(cudaMemcpyAsync(p, z, sizeof(TS) * nreal, cudaMemcpyDeviceToDevice, st));   // p0 = z0
       SOLVE_CUDA(sc_zero(c, 2, st));
       SOLVE_CUDA(dot2<TS>(c, rlo, z, nullptr, nreal, st));
@@ -563,7 +574,7 @@ int solve_impl(mspcg_ctx* c, const double* b_abi, double* x_abi, const mspcg_sol
         if (rnorm <= prm->tol * bnorm) { stt->converged = 1; break; }
       }
       if (rnorm > maxr) maxr = rnorm;
-      if (prm->use_precond) { SOLVE_CUDA(precond_any(c, rlo, z, sp, prm->n_inner, st)); stt->inner_applies += (long)prm->n_inner * c->lat.nblk; }
+      if (prm->use_precond) { SOLVE_CUDA(precond_any(c, rlo, z, sp, prm->n_inner, prm->use_reduced_ls != 0, st)); stt->inner_applies += (long)prm->n_inner * c->lat.nblk; }
       SOLVE_CUDA(sc_zero(c, 2, st));
       SOLVE_CUDA(dot2<TS>(c, z, rlo, Ap, nreal, st));
       SOLVE_CUDA(sc_read(c, 2, st));
@@ -643,7 +654,7 @@ int mspcg_set_reduced_ls(mspcg_ctx* ctx, int Ls_hat, const double* T_host, doubl
   if (!build_host_mats(ctx->hm_hat, Ls_hat, ctx->b, ctx->c, ctx->M5, ctx->mf)) return fail(ctx, MSPCG_EINVAL, "singular M5 at Ls_hat");
   ctx->Ls_hat = Ls_hat; ctx->mu_shift = mu;
   ctx->T_host.assign(T_host, T_host + (size_t)4 * Ls_hat * 4 * ctx->Ls * 2);
-  return fail(ctx, MSPCG_EINVAL, "reduced-Ls apply is not built yet (SURVEY 8(a) A10)");
+  return MSPCG_OK;
 }
 
 int mspcg_workspace_bytes(mspcg_ctx* ctx, int outer_prec, int inner_prec, int recon, size_t* bytes) {
@@ -676,6 +687,11 @@ int mspcg_set_workspace(mspcg_ctx* ctx, void* workspace_dev, size_t bytes, void*
   CUDA_OK(ctx, cudaStreamSynchronize(st));
   CUDA_OK(ctx, upload_mats<double>(ctx->md, ctx->hm, st)); CUDA_OK(ctx, upload_mats<float>(ctx->mf32, ctx->hm, st));
   CUDA_OK(ctx, upload_frags(ctx->mfr, ctx->hm, ctx->Ls, st));
+  if (ctx->Ls_hat) {
+    CUDA_OK(ctx, upload_mats<double>(ctx->md_hat, ctx->hm_hat, st)); CUDA_OK(ctx, upload_mats<float>(ctx->mf32_hat, ctx->hm_hat, st));
+    CUDA_OK(ctx, upload_frags(ctx->mfr_hat, ctx->hm_hat, ctx->Ls_hat, st));
+    CUDA_OK(ctx, up(ctx->Tm, ctx->T_host, st)); CUDA_OK(ctx, cudaStreamSynchronize(st));
+  }
   if (!ctx->sc_host) CUDA_OK(ctx, cudaMallocHost(&ctx->sc_host, sizeof(double) * 16));
   { int dev = 0, n = 0;
     if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0) ctx->num_sms = n; }
@@ -727,13 +743,13 @@ int mspcg_apply_precond(mspcg_ctx* ctx, const void* r_dev, void* z_dev, int io_p
                         int use_reduced, void* stream) {
   int rc = check_ready(ctx, true); if (rc) return rc;
   if (!r_dev || !z_dev || n_inner < 1 || n_inner > KMAX || !prec_ok(io_prec)) return fail(ctx, MSPCG_EINVAL, "bad argument (1 <= n_inner <= %d)", KMAX);
-  if (use_reduced) return fail(ctx, MSPCG_EINVAL, "reduced-Ls apply is not built yet (SURVEY 8(a) A10)");
+  if (use_reduced && !ctx->Ls_hat) return fail(ctx, MSPCG_EINVAL, "use_reduced without mspcg_set_reduced_ls");
   cudaStream_t st = (cudaStream_t)stream;
   if (layout == MSPCG_LAYOUT_NATIVE) {
-    CUDA_OK(ctx, precond_any(ctx, r_dev, z_dev, io_prec, n_inner, st));
+    CUDA_OK(ctx, precond_any(ctx, r_dev, z_dev, io_prec, n_inner, use_reduced != 0, st));
   } else {
     CUDA_OK(ctx, pack_any(ctx, (const double*)r_dev, ctx->stage_in, io_prec, 1, st));
-    CUDA_OK(ctx, precond_any(ctx, ctx->stage_in, ctx->stage_out, io_prec, n_inner, st));
+    CUDA_OK(ctx, precond_any(ctx, ctx->stage_in, ctx->stage_out, io_prec, n_inner, use_reduced != 0, st));
     CUDA_OK(ctx, pack_any(ctx, (double*)z_dev, ctx->stage_out, io_prec, 0, st));
   }
   return MSPCG_OK;
@@ -782,7 +798,7 @@ int mspcg_solve(mspcg_ctx* ctx, const double* b_dev, double* x_dev, const mspcg_
   int rc = check_ready(ctx, true); if (rc) return rc;
   if (!b_dev || !x_dev || !params || !stats) return fail(ctx, MSPCG_EINVAL, "null argument");
   if (params->use_precond && (params->n_inner < 1 || params->n_inner > KMAX)) return fail(ctx, MSPCG_EINVAL, "bad n_inner");
-  if (params->use_reduced_ls) return fail(ctx, MSPCG_EINVAL, "reduced-Ls apply is not built yet (SURVEY 8(a) A10)");
+  if (params->use_reduced_ls && !(params->use_precond && ctx->Ls_hat)) return fail(ctx, MSPCG_EINVAL, "use_reduced_ls needs use_precond and mspcg_set_reduced_ls");
   if (!full_buf(ctx, params->sloppy_prec)) return fail(ctx, MSPCG_EINVAL, "sloppy_prec not configured");
   cudaStream_t st = (cudaStream_t)stream;
   if (params->sloppy_prec == MSPCG_F64) return solve_impl<double>(ctx, b_dev, x_dev, params, stats, st);

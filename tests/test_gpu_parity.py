@@ -207,3 +207,50 @@ def test_error_codes():
         Mspcg((4, 4, 4, 5), 8, 1.5, 0.5, 1.8, 0.01)
     with pytest.raises(MspcgError):
         Mspcg((4, 4, 4, 4), 8, 1.5, 0.5, 1.8, 0.01, (3, 2, 2, 2))
+
+
+# ---- reduced-Ls preconditioner (eq. 19-21) against oracle/reduced_ls.py -----------
+def _reduced_setup(dims, Ls, Lh, block, mu, inner, outer=F64, seed=21):
+    import torch
+    from oracle import Oracle, reduced_ls
+    U = synth.gauge_natural_to_abi(synth.random_su3_links(dims, 0.3, 5), dims)
+    hat = Oracle(dims, Lh, MOB["b"], MOB["c"], MOB["M5"], 0.02, block)
+    hat.load_gauge(U, -1)
+    full = Oracle(dims, Ls, MOB["b"], MOB["c"], MOB["M5"], 0.02, block)
+    rng = np.random.default_rng(seed)
+    T = reduced_ls.initial_T(Ls, Lh) + 0.2 * (rng.standard_normal((Lh, 4, Ls, 4)) + 1j * rng.standard_normal((Lh, 4, Ls, 4)))
+    pre = reduced_ls.ReducedLsPrecond(hat.precond_obj(), T, mu)
+    g = Mspcg(dims, Ls, MOB["b"], MOB["c"], MOB["M5"], 0.02, block)
+    g.set_reduced_ls(Lh, reduced_ls.T_to_abi(T), mu)
+    g.configure(outer, inner, 18)
+    g.load_gauge(U, -1)
+    return full, pre, g, torch
+
+
+@pytest.mark.parametrize("dims,Ls,Lh,block", [((4, 4, 4, 4), 8, 4, (2, 2, 4, 4)), ((4, 4, 2, 6), 12, 6, (2, 2, 2, 6)),
+                                              ((4, 2, 4, 4), 6, 6, (2, 2, 2, 2))])
+def test_reduced_ls_precond_fp64(dims, Ls, Lh, block):
+    full, pre, g, torch = _reduced_setup(dims, Ls, Lh, block, 0.4, F64)
+    r = synth.gaussian_spinor_abi(dims, Ls, 23)
+    ref = full.pack(pre(full.unpack(r), 3))
+    z = g.apply_precond(dev(torch, r), 3, F64, use_reduced=1).cpu().numpy()
+    assert rel(z, ref) <= 1e-9
+    # the full-Ls preconditioner of the same context is untouched by set_reduced_ls
+    ora = OracleC(dims, Ls, MOB["b"], MOB["c"], MOB["M5"], 0.02, block)
+    ora.load_gauge(synth.gauge_natural_to_abi(synth.random_su3_links(dims, 0.3, 5), dims), -1)
+    assert rel(g.apply_precond(dev(torch, r), 3, F64).cpu().numpy(), ora.apply_precond(r, 3)) <= 1e-9
+
+
+def test_reduced_ls_precond_fp16_and_solve():
+    dims, Ls, Lh, block = (4, 4, 4, 8), 8, 4, (4, 4, 4, 4)
+    full, pre, g, torch = _reduced_setup(dims, Ls, Lh, block, 0.5, F16, outer=F32)
+    r = synth.gaussian_spinor_abi(dims, Ls, 25)
+    ref = full.pack(pre(full.unpack(r), 4))
+    z = g.apply_precond(dev(torch, r), 4, F64, use_reduced=1).cpu().numpy()
+    assert rel(z, ref) <= 2e-2
+    # MSPCG with the reduced-Ls preconditioner converges to the solution of the same system
+    ora = OracleC(dims, Ls, MOB["b"], MOB["c"], MOB["M5"], 0.02, block)
+    ora.load_gauge(synth.gauge_natural_to_abi(synth.random_su3_links(dims, 0.3, 5), dims), -1)
+    x_ref, _ = ora.solve(r, tol=1e-11)
+    x, st = g.solve(dev(torch, r), tol=1e-10, use_precond=True, n_inner=4, sloppy_prec=F32, use_reduced_ls=True)
+    assert st["rc"] == 0 and st["true_res"] <= 1e-10 and rel(x.cpu().numpy(), x_ref) <= 1e-8
