@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <type_traits>
@@ -77,6 +78,8 @@ struct mspcg_ctx {
   void *in_r = nullptr, *in_p = nullptr, *in_q = nullptr, *in_x = nullptr;   // inner CG vectors [V5h]
   double *rho = nullptr, *pq = nullptr; float* scale = nullptr; double* sc = nullptr;  // device scalars
   double* Tm = nullptr;          // device copy of the reduced-Ls transfer matrix T_host (A10)
+  __half *Bfwd = nullptr, *Bbwd = nullptr;   // fp16 B-operand images of T and T^dag for the tcgen05 transfer kernels
+  bool transfer_tc = true;       // use them when (Ls, Ls_hat) is a compiled pair and the inner storage is fp16
   double* sc_host = nullptr;     // pinned
   double *v_b = nullptr, *v_xhi = nullptr, *v_rhi = nullptr, *v_t64 = nullptr;   // solver, fp64 native
   void *v_xlo = nullptr, *v_rlo = nullptr, *v_p = nullptr, *v_Ap = nullptr, *v_z = nullptr;  // solver, sloppy
@@ -149,7 +152,7 @@ void carve(mspcg_ctx* c, Arena& a) {
   if (c->Ls_hat) { carve_mats(a, c->md_hat, c->Ls_hat); carve_mats(a, c->mf32_hat, c->Ls_hat); carve_frags(a, c->mfr_hat); }
   c->rho = a.take<double>((size_t)(KMAX + 1) * L.nblk); c->pq = a.take<double>((size_t)KMAX * L.nblk);
   c->scale = a.take<float>(L.nblk); c->sc = a.take<double>(16);
-  if (c->Ls_hat) c->Tm = a.take<double>((size_t)4 * c->Ls_hat * 4 * c->Ls * 2);
+  if (c->Ls_hat) { size_t nt = (size_t)4 * c->Ls_hat * 4 * c->Ls; c->Tm = a.take<double>(nt * 2); c->Bfwd = a.take<__half>(nt * 4); c->Bbwd = a.take<__half>(nt * 4); }
   carve_op(a, c->full64, L.full, MSPCG_F64, 18, c->Ls);
   if (c->outer_prec != MSPCG_F64) carve_op(a, c->fullS, L.full, c->outer_prec, c->recon, c->Ls);
   carve_op(a, c->blkI, L.blk, c->inner_prec, c->inner_prec == MSPCG_F64 ? 18 : c->recon, c->Ls);
@@ -316,6 +319,28 @@ cudaError_t convert_any(mspcg_ctx* c, const void* a, int pa, void* b, int pb, lo
 }
 
 // ---------------------------------------------------------------------------------------- the preconditioner (A7, A8)
+// tcgen05 transfer kernels (transfer_tc.cuh) for the compiled (Ls, Ls_hat) pairs; false = not available, use the generic ones.
+template <typename TIO>
+bool launch_transfer_tc(mspcg_ctx* c, bool forward, const TransferArgs& ta, int Ls, int Lh, int nblk, cudaStream_t st) {
+  dim3 grid((unsigned)((ta.n_sites + tc::TILE - 1) / tc::TILE), nblk);
+#define TT(LSV, LHV)                                                                                                     \
+  if (Ls == LSV && Lh == LHV) {                                                                                          \
+    static bool attr = false;                                                                                            \
+    if (!attr) {                                                                                                         \
+      cudaFuncSetAttribute(k_reduce_begin_tc<TIO, LSV, LHV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TransferCfg<LSV, LHV>::SMEM); \
+      cudaFuncSetAttribute(k_reduce_end_tc<TIO, LSV, LHV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TransferCfg<LHV, LSV>::SMEM);   \
+      attr = true;                                                                                                       \
+    }                                                                                                                    \
+    if (forward) k_reduce_begin_tc<TIO, LSV, LHV><<<grid, 128, TransferCfg<LSV, LHV>::SMEM, st>>>(ta);                   \
+    else k_reduce_end_tc<TIO, LSV, LHV><<<grid, 128, TransferCfg<LHV, LSV>::SMEM, st>>>(ta);                             \
+    return true;                                                                                                         \
+  }
+  TT(8, 4) TT(12, 6) TT(12, 8) TT(16, 8) TT(16, 12)
+#undef TT
+  return false;
+}
+template <> bool launch_transfer_tc<__half>(mspcg_ctx*, bool, const TransferArgs&, int, int, int, cudaStream_t) { return false; }
+
 // LS is the fifth-dimension extent of the inner iteration: Ls, or Ls_hat when `reduced` (then the right-hand side is
 // T r, the operator is built from the Ls_hat matrices, and z = T^dag x + mu r; eq. 19-21).
 template <typename TIO, typename T, int LS>
@@ -337,7 +362,14 @@ cudaError_t precond_impl(mspcg_ctx* c, const TIO* r_in, TIO* z_out, int k, bool 
   }
   T *r = (T*)c->in_r, *p = (T*)c->in_p, *q = (T*)c->in_q; TX* x = (TX*)c->in_x;
   { TimedLaunch tl(c, KIND_BLAS, st);
-    if (reduced) k_reduce_begin<TIO, T><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(r_in, r, g.nE0, c->Ls, LS, c->Tm, scale, c->rho);
+    bool done = false;
+    if (reduced && sizeof(T) == 2 && c->transfer_tc) {
+      TransferArgs ta; memset(&ta, 0, sizeof(ta));
+      ta.in = r_in; ta.out = r; ta.Bimg = c->Bfwd; ta.n_sites = g.nE0; ta.scale = scale; ta.rho0 = c->rho;
+      done = launch_transfer_tc<TIO>(c, true, ta, c->Ls, LS, nblk, st);
+    }
+    if (done) {}
+    else if (reduced) k_reduce_begin<TIO, T><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(r_in, r, g.nE0, c->Ls, LS, c->Tm, scale, c->rho);
     else k_pre_begin<TIO, T><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(r_in, r, g.nE0, LS, scale, c->rho); }
   c->launches++;
   for (int it = 0; it < k; it++) {
@@ -351,7 +383,13 @@ cudaError_t precond_impl(mspcg_ctx* c, const TIO* r_in, TIO* z_out, int k, bool 
   }
   if (reduced) {
     { TimedLaunch tl(c, KIND_BLAS, st);
-      k_reduce_end<TX, TIO><<<grid_sites(g.nE0, c->Ls, nblk), 128, 0, st>>>(x, r_in, z_out, g.nE0, c->Ls, LS, c->Tm, scale, c->mu_shift); }
+      bool done = false;
+      if (sizeof(T) == 2 && c->transfer_tc) {
+        TransferArgs ta; memset(&ta, 0, sizeof(ta));
+        ta.in = x; ta.rin = r_in; ta.out = z_out; ta.Bimg = c->Bbwd; ta.n_sites = g.nE0; ta.scale = scale; ta.mu = c->mu_shift;
+        done = launch_transfer_tc<TIO>(c, false, ta, c->Ls, LS, nblk, st);
+      }
+      if (!done) k_reduce_end<TX, TIO><<<grid_sites(g.nE0, c->Ls, nblk), 128, 0, st>>>(x, r_in, z_out, g.nE0, c->Ls, LS, c->Tm, scale, c->mu_shift); }
     c->launches++;
   }
   return cudaPeekAtLastError();
@@ -618,6 +656,7 @@ int mspcg_create(mspcg_ctx** out, int Lx, int Ly, int Lz, int Lt, int Ls, double
   const int L[4] = {Lx, Ly, Lz, Lt}, B[4] = {Bx, By, Bz, Bt};
   if (!build_lattice(ctx->lat, L, B)) { delete ctx; return MSPCG_EINVAL; }
   ctx->Ls = Ls; ctx->b = b; ctx->c = c; ctx->M5 = M5; ctx->mf = mf;
+  { const char* e = getenv("MSPCG_TRANSFER_TC"); if (e && e[0] == '0') ctx->transfer_tc = false; }   // debugging switch: generic transfer kernels
   ctx->alpha = b * (4.0 - M5) + 1.0; ctx->beta = c * (4.0 - M5) - 1.0;
   if (!build_host_mats(ctx->hm, Ls, b, c, M5, mf)) { delete ctx; return MSPCG_EINVAL; }
   *out = ctx;
@@ -691,6 +730,22 @@ int mspcg_set_workspace(mspcg_ctx* ctx, void* workspace_dev, size_t bytes, void*
     CUDA_OK(ctx, upload_mats<double>(ctx->md_hat, ctx->hm_hat, st)); CUDA_OK(ctx, upload_mats<float>(ctx->mf32_hat, ctx->hm_hat, st));
     CUDA_OK(ctx, upload_frags(ctx->mfr_hat, ctx->hm_hat, ctx->Ls_hat, st));
     CUDA_OK(ctx, up(ctx->Tm, ctx->T_host, st)); CUDA_OK(ctx, cudaStreamSynchronize(st));
+    { // B-operand images (UMMA canonical K-major, no swizzle: element (n, k) at (n/8)*KG*64 + (k/8)*64 + (n%8)*8 + k%8 halves)
+      const int Ls = ctx->Ls, Lh = ctx->Ls_hat;
+      auto Tc = [&](int ah, int m, int s, int n, int ri) { return ctx->T_host[((((size_t)ah * 4 + m) * (4 * Ls)) + s * 4 + n) * 2 + ri]; };
+      auto put = [&](std::vector<__half>& img, int KG, int n, int k, double v) { img[(size_t)(n / 8) * KG * 64 + (size_t)(k / 8) * 64 + (n % 8) * 8 + (k % 8)] = __float2half_rn((float)v); };
+      std::vector<__half> f((size_t)64 * Ls * Lh), b((size_t)64 * Ls * Lh);
+      for (int ah = 0; ah < Lh; ah++) for (int m = 0; m < 4; m++) for (int s = 0; s < Ls; s++) for (int n = 0; n < 4; n++) {
+        const double tr = Tc(ah, m, s, n, 0), ti = Tc(ah, m, s, n, 1);
+        // forward: row (ah, sp, hi, ri') with m = 2*hi + sp (fp16 fragment order), column (s, n, ri)
+        const int rowf = ah * 8 + ((m & 1) * 2 + (m >> 1)) * 2, colf = s * 8 + n * 2;
+        put(f, Ls, rowf, colf, tr); put(f, Ls, rowf, colf + 1, -ti); put(f, Ls, rowf + 1, colf, ti); put(f, Ls, rowf + 1, colf + 1, tr);
+        // backward (conj T): row (s, n, ri'), column (ah, m, ri)
+        const int rowb = s * 8 + n * 2, colb = ah * 8 + m * 2;
+        put(b, Lh, rowb, colb, tr); put(b, Lh, rowb, colb + 1, ti); put(b, Lh, rowb + 1, colb, -ti); put(b, Lh, rowb + 1, colb + 1, tr);
+      }
+      CUDA_OK(ctx, up(ctx->Bfwd, f, st)); CUDA_OK(ctx, up(ctx->Bbwd, b, st)); CUDA_OK(ctx, cudaStreamSynchronize(st));
+    }
   }
   if (!ctx->sc_host) CUDA_OK(ctx, cudaMallocHost(&ctx->sc_host, sizeof(double) * 16));
   { int dev = 0, n = 0;

@@ -254,3 +254,23 @@ def test_reduced_ls_precond_fp16_and_solve():
     x_ref, _ = ora.solve(r, tol=1e-11)
     x, st = g.solve(dev(torch, r), tol=1e-10, use_precond=True, n_inner=4, sloppy_prec=F32, use_reduced_ls=True)
     assert st["rc"] == 0 and st["true_res"] <= 1e-10 and rel(x.cpu().numpy(), x_ref) <= 1e-8
+
+
+@pytest.mark.parametrize("dims,Ls,Lh,block", [((4, 4, 4, 8), 8, 4, (4, 4, 4, 4)), ((8, 4, 4, 6), 12, 6, (4, 4, 4, 6)),
+                                              ((4, 4, 6, 8), 16, 8, (2, 4, 6, 4))])
+def test_reduced_ls_transfer_on_tcgen05_matches_generic_kernels(dims, Ls, Lh, block, monkeypatch):
+    """The tcgen05 transfer kernels (fp16 operands, fp32 accumulation in tensor memory) against the generic CUDA-core
+    ones (MSPCG_TRANSFER_TC=0) and against the oracle; tile tails: nE0 per block is not a multiple of 128."""
+    r = synth.gaussian_spinor_abi(dims, Ls, 27)
+    out = {}
+    for flag in ("1", "0"):
+        monkeypatch.setenv("MSPCG_TRANSFER_TC", flag)
+        full, pre, g, torch = _reduced_setup(dims, Ls, Lh, block, 0.3, F16, outer=F32)
+        out[flag] = g.apply_precond(dev(torch, r), 4, F64, use_reduced=1).cpu().numpy()
+        nat = g.pack(dev(torch, r), F32)
+        out[flag + "f32"] = g.unpack(g.apply_precond(nat, 4, F32, LAYOUT_NATIVE, use_reduced=1), F32).cpu().numpy()
+        g.close()
+    ref = full.pack(pre(full.unpack(r), 4))
+    for k in out:
+        assert rel(out[k], ref) <= 2e-2
+    assert rel(out["1"], out["0"]) <= 5e-3 and rel(out["1f32"], out["0f32"]) <= 5e-3
