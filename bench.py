@@ -146,6 +146,17 @@ def ncu_traffic():
     return json.load(open(p)) if os.path.exists(p) else {}
 
 
+def initial_T_abi(Ls, Lh):
+    """Untrained transfer matrix (reading R20): spin identity, keeps the Lh/2 slices next to each domain wall.
+    float64 [4*Lh][4*Ls][re,im] as include/mspcg.h asks."""
+    T = np.zeros((Lh, 4, Ls, 4, 2))
+    for a in range(Lh):
+        s = a if a < Lh // 2 else Ls - Lh + a
+        for m in range(4):
+            T[a, m, s, m, 0] = 1.0
+    return T.reshape(-1)
+
+
 def make_inputs(cfg):
     dims, Ls = cfg["dims"], cfg["Ls"]
     U = synth.gauge_natural_to_abi(synth.random_su3_links(dims, cfg["eps"], cfg["gauge_seed"]), dims)
@@ -188,6 +199,8 @@ def run_ours(args):
     dims, Ls, block, k = cfg["dims"], cfg["Ls"], cfg["block"], cfg["n_inner"]
     U, src = make_inputs(cfg)
     g = Mspcg(dims, Ls, cfg["b"], cfg["c"], cfg["M5"], cfg["mf"], block)
+    if args.reduced:   # profiling aid: the step's preconditioner becomes the reduced-Ls one (untrained T, eq. 20-21)
+        g.set_reduced_ls(args.reduced, initial_T_abi(Ls, args.reduced), 0.5)
     ws = g.configure(F32, F16, 18)
     g.load_gauge(U, -1)
     geo = g.geometry()
@@ -196,7 +209,7 @@ def run_ours(args):
     z32, q32 = g.new_native(F32), g.new_native(F32)
 
     def step():
-        g.apply_precond(r32, k, F32, LAYOUT_NATIVE, out=z32)
+        g.apply_precond(r32, k, F32, LAYOUT_NATIVE, out=z32, use_reduced=1 if args.reduced else 0)
         g.apply_MdagM(r32, F32, LAYOUT_NATIVE, out=q32)
 
     # ---- work model of one step
@@ -264,16 +277,21 @@ def run_ours(args):
             ent["frac"] = ent["GBps"] / peak
         kern[name] = ent
     dom = max((n for n in kern if n in alg), key=lambda n: tm[n]["ms"])
-    traffic = ncu_traffic().get(dom)
+    prof = ncu_traffic()
+    traffic = prof.get(dom)
     roofline = dict(bound="hbm", kernel=dom, achieved=kern[dom]["GBps"], peak=peak, unit="GB/s", frac=kern[dom]["frac"],
                     traffic=traffic, peak_source=peak_src, alg_bytes_per_launch=kern[dom]["alg_bytes"],
-                    avg_launch_ms=kern[dom]["avg_ms"], share_of_step=kern[dom]["share"])
+                    avg_launch_ms=kern[dom]["avg_ms"], share_of_step=kern[dom]["share"],
+                    # utilisation of the tensor pipe by the SU(3) and M5^-1 contractions of this kernel, from the committed
+                    # ncu --set full capture (profiles/traffic.json), not measured in this run
+                    tensor_pipe_pct_ncu=(prof.get("tensor_pipe_pct") or {}).get(dom))
 
     out = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
                ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f16/f32",
                data="synthetic", impl="ours",
                config=dict(workload=f"{args.workload}: {dims[0]}x{dims[1]}x{dims[2]}x{dims[3]} Ls={Ls} blocks {block} "
-                                    f"M_pre(k={k}, fp16 storage/fp32 math) + DdagD(fp32)", parallelism="replicas only",
+                                    f"M_pre(k={k}, fp16 storage/fp32 math) + DdagD(fp32)" + (f" [reduced-Ls {args.reduced}: flop model of the full-Ls step, not a headline]" if args.reduced else ""),
+                           parallelism="replicas only",
                            l2="working set of a step %.0f MiB > 126 MB L2 (no flush)" % (ws / 2**20), workspace_bytes=ws,
                            flops_per_step=flops_step, alg_bytes_per_step=by_pre + by_op),
                gpu_launches=launches, clocks=clocks, e2e=e2e, roofline=roofline, kernels=kern,
@@ -323,6 +341,21 @@ def extras(torch, g, cfg, U, src, d_src, geo, peak, args):
     ex["solve_tol1e-10_fp32outer_fp16inner"] = sol
     del x
     g.close()
+    torch.cuda.empty_cache()
+    # reduced-Ls preconditioner with the UNTRAINED transfer matrix: cost per application and its
+    # effect on the outer iteration count (the trained T of eq. 22 is a set-up step)
+    Lh = cfg.get("Ls_hat", Ls // 2)
+    gr = Mspcg(dims, Ls, cfg["b"], cfg["c"], cfg["M5"], cfg["mf"], block)
+    gr.set_reduced_ls(Lh, initial_T_abi(Ls, Lh), 0.5)
+    gr.configure(F32, F16, 18)
+    gr.load_gauge(U, -1)
+    v, o = gr.pack(d_src, F32), gr.new_native(F32)
+    ms = timed(torch, lambda: gr.apply_precond(v, k, F32, LAYOUT_NATIVE, out=o, use_reduced=1), steps, warm) / steps
+    x, s = gr.solve(d_src, tol=1e-10, max_iter=20000, use_precond=True, n_inner=k, sloppy_prec=F32, delta=0.1, use_reduced_ls=True)
+    ex["reducedLs%d_untrainedT_mu0.5" % Lh] = dict(Mpre_ms=ms, solve=dict(seconds=s["seconds"], outer_iters=s["iters"], reliable_updates=s["reliable_updates"],
+                                                   inner_applies=s["inner_applies"], true_res=s["true_res"], rc=s["rc"]))
+    del x, v, o
+    gr.close()
     torch.cuda.empty_cache()
     g2 = Mspcg(dims, Ls, cfg["b"], cfg["c"], cfg["M5"], cfg["mf"], block)
     g2.configure(F16, F64, 18)
@@ -402,6 +435,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C2", choices=sorted(synth.CONFIGS))
     ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--reduced", type=int, default=0, help="profiling aid: run the step with the reduced-Ls preconditioner at this Ls_hat")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
