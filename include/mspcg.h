@@ -96,9 +96,14 @@ int mspcg_apply_precond_host(mspcg_ctx* ctx, const double* r_host, double* z_hos
  * out is zero outside the block. */
 int mspcg_apply_A_block(mspcg_ctx* ctx, const double* in_dev, double* out_dev, int block, int prec, void* stream);
 
-/* Reduced-Ls preconditioner: Ls_hat in the compiled set, T_host[4*Ls_hat][4*Ls][re,im] (HOST,
- * row (s_hat,spin), column (s,spin); identity in colour and 4D site, eq. 21), shift mu (eq. 20).  Must be called
- * before mspcg_workspace_bytes. */
+/* Reduced-Ls preconditioner: Ls_hat in {4,6,8,12,16}, Ls_hat <= Ls; T_host[4*Ls_hat][4*Ls][re,im]
+ * (HOST, copied; row (s_hat,spin), column (s,spin); identity in colour and 4D site, eq. 21), shift mu (eq. 20).  The
+ * reduced operator uses the same b, c, M5, mf (reading R19).  Must be called before mspcg_workspace_bytes.  Afterwards
+ * use_reduced != 0 in mspcg_apply_precond / use_reduced_ls in mspcg_solve_params selects
+ *     z = T^dag CG_k[Mhat](T r) + mu r ;
+ * the full-Ls preconditioner of the same context stays available.  With fp16 inner storage and (Ls, Ls_hat) in
+ * {(8,4),(12,6),(12,8),(16,8),(16,12)} the two transfers run as tcgen05.mma contractions (fp16 operands, fp32
+ * accumulation), otherwise on the CUDA cores in fp64.  Errors: MSPCG_EINVAL (bad Ls_hat, null T, called too late). */
 int mspcg_set_reduced_ls(mspcg_ctx* ctx, int Ls_hat, const double* T_host, double mu);
 
 typedef struct {
