@@ -335,7 +335,7 @@ def extras(torch, g, cfg, U, src, d_src, geo, peak, args):
     # time to solution, plain CG vs MSPCG, sloppy fp32 + fp64 reliable updates, preconditioner fp16
     sol = {}
     for name, pre in (("CG", False), ("MSPCG", True)):
-        x, s = g.solve(d_src, tol=1e-10, max_iter=20000, use_precond=pre, n_inner=k, sloppy_prec=F32, delta=0.1)
+        x, s = g.solve(d_src, tol=1e-10, max_iter=200000, use_precond=pre, n_inner=k, sloppy_prec=F32, delta=0.1)
         sol[name] = dict(seconds=s["seconds"], outer_iters=s["iters"], reliable_updates=s["reliable_updates"],
                          inner_applies=s["inner_applies"], true_res=s["true_res"], rc=s["rc"])
     ex["solve_tol1e-10_fp32outer_fp16inner"] = sol
@@ -351,7 +351,7 @@ def extras(torch, g, cfg, U, src, d_src, geo, peak, args):
     gr.load_gauge(U, -1)
     v, o = gr.pack(d_src, F32), gr.new_native(F32)
     ms = timed(torch, lambda: gr.apply_precond(v, k, F32, LAYOUT_NATIVE, out=o, use_reduced=1), steps, warm) / steps
-    x, s = gr.solve(d_src, tol=1e-10, max_iter=20000, use_precond=True, n_inner=k, sloppy_prec=F32, delta=0.1, use_reduced_ls=True)
+    x, s = gr.solve(d_src, tol=1e-10, max_iter=200000, use_precond=True, n_inner=k, sloppy_prec=F32, delta=0.1, use_reduced_ls=True)
     ex["reducedLs%d_untrainedT_mu0.5" % Lh] = dict(Mpre_ms=ms, solve=dict(seconds=s["seconds"], outer_iters=s["iters"], reliable_updates=s["reliable_updates"],
                                                    inner_applies=s["inner_applies"], true_res=s["true_res"], rc=s["rc"]))
     del x, v, o

@@ -16,8 +16,12 @@ Pins (tests/test_oracle_reduced_ls.py): Ls_hat = Ls, T = 1, mu = 0 reproduces th
 the mu term is exactly mu*r; T = a cyclic slice permutation, T = 1 (x) gamma5, T = i*1 and T = a slice selection
 each against the same map written with explicit array indexing (they fail if T and T^dag are exchanged, if the
 conjugate is dropped, or if the spin and slice indices are transposed).  initial_T (reading R20: the paper does not
-give the starting point of the training) is a convention, not a result: parity unpinned.  The training of T
-(eq. 22) is not implemented in the oracle.
+give the starting point of the training) is a convention, not a result: parity unpinned.
+
+Training of T (eq. 22; reading R20): chi2, its gradient with respect to conj(T) and one
+line-search step with momentum.  Pins: chi2 = 0 at Ls_hat = Ls, T = 1, mu = 0 with a converged block solve
+(PAPER.md:322); the analytic gradient against central finite differences of chi2 in random directions (with a
+converged, hence linear and Hermitian, Mhat^-1); the exact quartic line search against a brute-force scan.
 """
 from __future__ import annotations
 
@@ -63,3 +67,63 @@ class ReducedLsPrecond:
 
     def __call__(self, r, k):
         return apply_Tdag(self.T, self.pre_hat(apply_T(self.T, r), k)) + self.mu * r
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# eq. 22:  chi2(T) = sum_i | M (T^dag Ahat T + mu) v_i - v_i |^2
+#   M    = the full-Ls block operator (+)_s A_s (Hermitian),  M_apply(w) -> M w
+#   Ahat = Mhat^-1 = the fixed-count block CG at Ls_hat,      Ahat_apply(r_hat) -> z_hat
+# Reading R20: for the derivative Ahat is treated as a fixed Hermitian linear operator.  With
+#   w = (T^dag Ahat T + mu) v,  e = M w - v,  g = M e,  a = Ahat T v,  c = Ahat T g:
+#   d chi2 = 2 Re sum_i [ <c_i, dT v_i> + <a_i, dT g_i> ]   =>   G = d chi2 / d conj(T) = sum_i (c_i v_i^dag + a_i g_i^dag)
+# (outer products summed over 4D sites and colour; G has the shape of T).
+# ---------------------------------------------------------------------------------------------------------------
+def outer_T(x_hat, y):
+    """sum over sites and colour of x_hat[a, ..., m, c] conj(y[b, ..., n, c]) -> [a, m, b, n]."""
+    return np.einsum("atzyxmc,btzyxnc->ambn", x_hat, np.conj(y))
+
+
+def chi2_terms(M_apply, Ahat_apply, T, mu, v):
+    a = Ahat_apply(apply_T(T, v))
+    w = apply_Tdag(T, a) + mu * v
+    e = M_apply(w) - v
+    return a, w, e
+
+
+def chi2(M_apply, Ahat_apply, T, mu, vs):
+    return float(sum(np.vdot(e, e).real for e in (chi2_terms(M_apply, Ahat_apply, T, mu, v)[2] for v in vs)))
+
+
+def chi2_and_gradient(M_apply, Ahat_apply, T, mu, vs):
+    val, G = 0.0, np.zeros_like(T)
+    for v in vs:
+        a, w, e = chi2_terms(M_apply, Ahat_apply, T, mu, v)
+        val += float(np.vdot(e, e).real)
+        g = M_apply(e)
+        c = Ahat_apply(apply_T(T, g))
+        G += outer_T(c, v) + outer_T(a, g)
+    return val, G
+
+
+def quartic_minimum(etas, vals):
+    """chi2(T + eta P) is a quartic in eta when Ahat is linear: fit it through five evaluations and return the real
+    stationary point with the smallest fitted value ("line search")."""
+    coef = np.polyfit(np.asarray(etas, dtype=np.float64), np.asarray(vals, dtype=np.float64), 4)
+    roots = np.roots(np.polyder(coef))
+    cand = [r.real for r in roots if abs(r.imag) <= 1e-9 * max(1.0, abs(r.real))]
+    if not cand:
+        return float(etas[int(np.argmin(vals))])
+    return float(min(cand, key=lambda x: np.polyval(coef, x)))
+
+
+def train_step(M_apply, Ahat_apply, T, mu, vs, direction_prev=None, momentum=0.0, eta0=None):
+    """One step: P = -G + momentum * P_prev; five evaluations at eta0 * (0, 1/2, 1, 3/2, 2); T <- T + eta* P.
+    eta0 defaults to chi2 / |G|^2 (the Newton-like scale of a quadratic).  Returns (T_new, P, chi2_before, eta*)."""
+    val, G = chi2_and_gradient(M_apply, Ahat_apply, T, mu, vs)
+    P = -G if direction_prev is None else -G + momentum * direction_prev
+    if eta0 is None:
+        eta0 = val / float(np.vdot(G, G).real)
+    etas = [0.0, 0.5 * eta0, eta0, 1.5 * eta0, 2.0 * eta0]
+    vals = [val] + [chi2(M_apply, Ahat_apply, T + h * P, mu, vs) for h in etas[1:]]
+    eta = quartic_minimum(etas, vals)
+    return T + eta * P, P, val, eta

@@ -85,3 +85,49 @@ def test_reduced_pcg_reaches_the_same_solution():
     x0, s0 = solvers.pcg(A, r, None, 1e-9)
     x1, s1 = solvers.pcg(A, r, lambda v: pre(v, 3), 1e-9)
     assert rel(x1, x0) <= 1e-7 and s1["converged"]
+
+
+# ---- training of T (eq. 22; reading R20) ------------------------------------------------------------
+def _train_setup(Ls_hat, k):
+    dims, block = (2, 2, 2, 4), (2, 2, 2, 2)
+    full, hat, r = _setup(Ls_hat, dims, block)
+    Pf, Ph = full.precond_obj(), hat.precond_obj()
+
+    def M_apply(w):   # (+)_s A_s w
+        out = np.zeros_like(w)
+        for o in Pf.origins:
+            out += Pf.apply_A_block(o, w)
+        return out
+    vs = [r]
+    return M_apply, (lambda rh: Ph(rh, k)), vs
+
+
+def test_chi2_vanishes_for_identity_T():
+    """Ls_hat = Ls => Mhat = M, optimal T = 1, optimal chi2 = 0 (mu = 0, converged block solve)."""
+    M_apply, Ahat, vs = _train_setup(LS, 160)
+    c0 = reduced_ls.chi2(M_apply, Ahat, reduced_ls.initial_T(LS, LS), 0.0, vs)
+    norm = sum(np.vdot(v, v).real for v in vs)
+    assert c0 <= 1e-16 * norm
+    # and it does not vanish away from it
+    assert reduced_ls.chi2(M_apply, Ahat, 0.9 * reduced_ls.initial_T(LS, LS), 0.0, vs) > 1e-3 * norm
+
+
+def test_gradient_against_finite_differences_and_line_search():
+    M_apply, Ahat, vs = _train_setup(2, 120)      # converged CG: Ahat is linear and Hermitian, as R20 assumes
+    rng = np.random.default_rng(8)
+    T = reduced_ls.initial_T(LS, 2) + 0.1 * (rng.standard_normal((2, 4, LS, 4)) + 1j * rng.standard_normal((2, 4, LS, 4)))
+    mu = 0.3
+    val, G = reduced_ls.chi2_and_gradient(M_apply, Ahat, T, mu, vs)
+    assert abs(val - reduced_ls.chi2(M_apply, Ahat, T, mu, vs)) <= 1e-12 * val
+    for seed in (1,):
+        r2 = np.random.default_rng(seed)
+        dT = r2.standard_normal(T.shape) + 1j * r2.standard_normal(T.shape)
+        h = 1e-5
+        fd = (reduced_ls.chi2(M_apply, Ahat, T + h * dT, mu, vs) - reduced_ls.chi2(M_apply, Ahat, T - h * dT, mu, vs)) / (2 * h)
+        an = 2.0 * np.vdot(G, dT).real
+        assert abs(fd - an) <= 1e-6 * abs(an)
+    # the quartic through five points is exact for a linear Ahat: its minimum beats a brute-force scan along -G
+    T1, P, v0, eta = reduced_ls.train_step(M_apply, Ahat, T, mu, vs)
+    v1 = reduced_ls.chi2(M_apply, Ahat, T1, mu, vs)
+    scan = min(reduced_ls.chi2(M_apply, Ahat, T + x * eta * P, mu, vs) for x in (0.9, 1.1))
+    assert v1 < v0 and v1 <= scan * (1 + 1e-9)
