@@ -106,6 +106,24 @@ int mspcg_apply_A_block(mspcg_ctx* ctx, const double* in_dev, double* out_dev, i
  * accumulation), otherwise on the CUDA cores in fp64.  Errors: MSPCG_EINVAL (bad Ls_hat, null T, called too late). */
 int mspcg_set_reduced_ls(mspcg_ctx* ctx, int Ls_hat, const double* T_host, double mu);
 
+/* Replace T and mu of a context whose workspace is already set (HOST T as in mspcg_set_reduced_ls, same Ls_hat). */
+int mspcg_update_T(mspcg_ctx* ctx, const double* T_host, double mu, void* stream);
+
+/* Training of T (eq. 22; reading R20) -- a set-up step, not on the timed path.
+ *   chi2 = sum_i | M (T^dag Ahat T + mu) v_i - v_i |^2 ,   M = (+)_s A_s (full Ls),  Ahat = n_inner block-CG steps at Ls_hat,
+ *   grad = d chi2 / d conj(T) = sum_i (c_i v_i^dag + a_i g_i^dag)  with Ahat treated as a fixed Hermitian operator
+ *   (e = M w - v, g = M e, a = Ahat T v, c = Ahat T g), layout of T_host.
+ * v_dev: nvec DEVICE fp64 ABI vectors, contiguous (the paper uses residual vectors of a full-Ls MSPCG run).  chi2_host:
+ * HOST double; grad_host: HOST [4*Ls_hat][4*Ls][re,im] or NULL.  Needs inner_prec fp64 or fp32 (EINVAL for fp16: train in
+ * one context, use T in any).  Synchronous. */
+int mspcg_train_eval(mspcg_ctx* ctx, const double* v_dev, int nvec, int n_inner, double* chi2_host, double* grad_host, void* stream);
+/* n_steps of: P = -grad + momentum * P_prev; chi2 at eta0 * (0, 1/2, 1, 3/2, 2), eta0 = chi2 / |grad|^2; T += eta* P with eta*
+ * the minimiser of the quartic through the five values ("line search", "momentum method").  The context's T
+ * is updated; T_host_out (HOST, layout of T_host) receives it; chi2_history_host (HOST, n_steps + 1 doubles or NULL) the
+ * loss before every step and after the last. */
+int mspcg_train_T(mspcg_ctx* ctx, const double* v_dev, int nvec, int n_inner, int n_steps, double momentum, double* T_host_out,
+                  double* chi2_history_host, void* stream);
+
 typedef struct {
   double tol;          /* relative residual |r|/|b| (R15)                                                        */
   int max_iter;        /* outer iteration cap                                                                    */

@@ -23,7 +23,7 @@ SYMBOLS = [
     "mspcg_workspace_bytes", "mspcg_set_workspace", "mspcg_load_gauge", "mspcg_vec_bytes", "mspcg_pack",
     "mspcg_unpack", "mspcg_apply_MdagM", "mspcg_apply_precond", "mspcg_apply_MdagM_host",
     "mspcg_apply_precond_host", "mspcg_apply_A_block", "mspcg_set_reduced_ls", "mspcg_solve", "mspcg_launch_count",
-    "mspcg_timing", "mspcg_timing_read",
+    "mspcg_timing", "mspcg_timing_read", "mspcg_update_T", "mspcg_train_eval", "mspcg_train_T",
 ]
 
 
@@ -73,6 +73,9 @@ def load_library():
     L.mspcg_solve.argtypes = [vp, vp, vp, C.POINTER(SolveParams), C.POINTER(SolveStats), vp]
     L.mspcg_launch_count.argtypes = [vp]
     L.mspcg_launch_count.restype = C.c_long
+    L.mspcg_update_T.argtypes = [vp, dp, d, vp]
+    L.mspcg_train_eval.argtypes = [vp, vp, i, i, dp, dp, vp]
+    L.mspcg_train_T.argtypes = [vp, vp, i, i, i, d, dp, dp, vp]
     L.mspcg_timing.argtypes = [vp, i]
     L.mspcg_timing_read.argtypes = [vp, dp, C.POINTER(C.c_long)]
     _lib = L
@@ -159,6 +162,27 @@ class Mspcg:
         assert T.size == 4 * int(Ls_hat) * 4 * self.Ls * 2
         self._check(self.lib.mspcg_set_reduced_ls(self.h, int(Ls_hat), T.ctypes.data_as(C.POINTER(C.c_double)), float(mu)))
         self.Ls_hat = int(Ls_hat)
+
+    def update_T(self, T_abi, mu):
+        T = np.ascontiguousarray(T_abi, dtype=np.float64).reshape(-1)
+        self._check(self.lib.mspcg_update_T(self.h, T.ctypes.data_as(C.POINTER(C.c_double)), float(mu), self._stream()))
+
+    def train_eval(self, vs, n_inner, want_grad=True):
+        """chi2 of eq. 22 (and its gradient, layout of T_abi) for the current T; vs: torch fp64 CUDA tensor [nvec * nreal]."""
+        nvec = vs.numel() // self.nreal
+        chi2 = C.c_double()
+        G = np.zeros(4 * self.Ls_hat * 4 * self.Ls * 2)
+        gp = G.ctypes.data_as(C.POINTER(C.c_double)) if want_grad else None
+        self._check(self.lib.mspcg_train_eval(self.h, C.c_void_p(vs.data_ptr()), nvec, int(n_inner), C.byref(chi2), gp, self._stream()))
+        return chi2.value, (G if want_grad else None)
+
+    def train_T(self, vs, n_inner, n_steps, momentum=0.0):
+        nvec = vs.numel() // self.nreal
+        T = np.zeros(4 * self.Ls_hat * 4 * self.Ls * 2)
+        hist = np.zeros(n_steps + 1)
+        self._check(self.lib.mspcg_train_T(self.h, C.c_void_p(vs.data_ptr()), nvec, int(n_inner), int(n_steps), float(momentum),
+                                           T.ctypes.data_as(C.POINTER(C.c_double)), hist.ctypes.data_as(C.POINTER(C.c_double)), self._stream()))
+        return T, hist
 
     # ---- device set-up -----------------------------------------------------------------------------------------
     def _stream(self):

@@ -567,6 +567,55 @@ __global__ void k_reduce_end(const TX* __restrict__ xhat, const TIO* __restrict_
   store24<TIO>(z, t.gsite, t.s, Ls, o);
 }
 
+// Training of T (eq. 22, reading R20): G[a m, s n] += sum over sites and colour of
+// x[a, m, c] * conj(y[s, n, c]),  x an Ls_hat vector (TX), y an Ls vector (fp64).  One thread block per SPB sites,
+// both site columns staged in shared memory, thread e owns the entries e, e + blockDim, ... of the 4Lh x 4Ls matrix.
+template <typename TX>
+__global__ void k_outer_T(const TX* __restrict__ x, const double* __restrict__ y, long n_sites_total, int Ls, int Lh, int spb, double* __restrict__ G) {
+  extern __shared__ double osm[];
+  double* xs = osm;               // [Lh][24]
+  double* ys = osm + 24 * Lh;     // [Ls][24]
+  const int nent = 16 * Lh * Ls;
+  constexpr int MAXE = 8;         // entries per thread (16*16*16 / 512)
+  double accr[MAXE], acci[MAXE];
+#pragma unroll
+  for (int i = 0; i < MAXE; i++) { accr[i] = 0; acci[i] = 0; }
+  const long s0 = (long)blockIdx.x * spb;
+  for (int j = 0; j < spb; j++) {
+    const long site = s0 + j;
+    if (site >= n_sites_total) break;
+    __syncthreads();
+    for (int l = threadIdx.x; l < Lh + Ls; l += blockDim.x) {
+      if (l < Lh) { typename ST<TX>::C v[24]; load24<TX>(x, site, l, Lh, v);
+#pragma unroll
+        for (int k = 0; k < 24; k++) xs[l * 24 + k] = (double)v[k]; }
+      else { double v[24]; load24<double>(y, site, l - Lh, Ls, v);
+#pragma unroll
+        for (int k = 0; k < 24; k++) ys[(l - Lh) * 24 + k] = v[k]; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < MAXE; i++) {
+      const int e = threadIdx.x + i * blockDim.x;
+      if (e < nent) {
+        const int row = e / (4 * Ls), col = e - row * (4 * Ls);   // row = a*4 + m, col = s*4 + n
+        const double* xp = xs + (row >> 2) * 24 + (row & 3) * 6;
+        const double* yp = ys + (col >> 2) * 24 + (col & 3) * 6;
+#pragma unroll
+        for (int c = 0; c < 3; c++) {   // x * conj(y)
+          accr[i] += xp[2 * c] * yp[2 * c] + xp[2 * c + 1] * yp[2 * c + 1];
+          acci[i] += xp[2 * c + 1] * yp[2 * c] - xp[2 * c] * yp[2 * c + 1];
+        }
+      }
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < MAXE; i++) {
+    const int e = threadIdx.x + i * blockDim.x;
+    if (e < nent) { atomicAdd(G + 2 * e, accr[i]); atomicAdd(G + 2 * e + 1, acci[i]); }
+  }
+}
+
 // Same-precision flat kernels: one thread per 16-byte chunk.
 template <typename T> __device__ __forceinline__ void ldchunk(const T* base, long i, typename ST<T>::C* v) {
   typedef typename ST<T>::V V; V q = __ldg(reinterpret_cast<const V*>(base) + i); unpackV(q, v);

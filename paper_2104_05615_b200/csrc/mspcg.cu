@@ -78,6 +78,7 @@ struct mspcg_ctx {
   void *in_r = nullptr, *in_p = nullptr, *in_q = nullptr, *in_x = nullptr;   // inner CG vectors [V5h]
   double *rho = nullptr, *pq = nullptr; float* scale = nullptr; double* sc = nullptr;  // device scalars
   double* Tm = nullptr;          // device copy of the reduced-Ls transfer matrix T_host (A10)
+  double* Gdev = nullptr;        // gradient accumulator of the T training (A12)
   __half *Bfwd = nullptr, *Bbwd = nullptr;   // fp16 B-operand images of T and T^dag for the tcgen05 transfer kernels
   bool transfer_tc = true;       // use them when (Ls, Ls_hat) is a compiled pair and the inner storage is fp16
   double* sc_host = nullptr;     // pinned
@@ -152,7 +153,7 @@ void carve(mspcg_ctx* c, Arena& a) {
   if (c->Ls_hat) { carve_mats(a, c->md_hat, c->Ls_hat); carve_mats(a, c->mf32_hat, c->Ls_hat); carve_frags(a, c->mfr_hat); }
   c->rho = a.take<double>((size_t)(KMAX + 1) * L.nblk); c->pq = a.take<double>((size_t)KMAX * L.nblk);
   c->scale = a.take<float>(L.nblk); c->sc = a.take<double>(16);
-  if (c->Ls_hat) { size_t nt = (size_t)4 * c->Ls_hat * 4 * c->Ls; c->Tm = a.take<double>(nt * 2); c->Bfwd = a.take<__half>(nt * 4); c->Bbwd = a.take<__half>(nt * 4); }
+  if (c->Ls_hat) { size_t nt = (size_t)4 * c->Ls_hat * 4 * c->Ls; c->Tm = a.take<double>(nt * 2); c->Bfwd = a.take<__half>(nt * 4); c->Bbwd = a.take<__half>(nt * 4); c->Gdev = a.take<double>(nt * 2); }
   carve_op(a, c->full64, L.full, MSPCG_F64, 18, c->Ls);
   if (c->outer_prec != MSPCG_F64) carve_op(a, c->fullS, L.full, c->outer_prec, c->recon, c->Ls);
   carve_op(a, c->blkI, L.blk, c->inner_prec, c->inner_prec == MSPCG_F64 ? 18 : c->recon, c->Ls);
@@ -497,6 +498,27 @@ template <typename V> cudaError_t up(void* dst, const std::vector<V>& src, cudaS
   return cudaMemcpyAsync(dst, src.data(), src.size() * sizeof(V), cudaMemcpyHostToDevice, st);
 }
 
+// Device copies of the reduced-Ls transfer matrix: fp64 T for the generic kernels and the fp16 B-operand images of T and
+// T^dag for the tcgen05 kernels (UMMA canonical K-major, no swizzle: element (n, k) at (n/8)*KG*64 + (k/8)*64 + (n%8)*8 + k%8).
+int upload_T(mspcg_ctx* ctx, cudaStream_t st) {
+  CUDA_OK(ctx, up(ctx->Tm, ctx->T_host, st)); CUDA_OK(ctx, cudaStreamSynchronize(st));
+  const int Ls = ctx->Ls, Lh = ctx->Ls_hat;
+  auto Tc = [&](int ah, int m, int s, int n, int ri) { return ctx->T_host[((((size_t)ah * 4 + m) * (4 * Ls)) + s * 4 + n) * 2 + ri]; };
+  auto put = [&](std::vector<__half>& img, int KG, int n, int k, double v) { img[(size_t)(n / 8) * KG * 64 + (size_t)(k / 8) * 64 + (n % 8) * 8 + (k % 8)] = __float2half_rn((float)v); };
+  std::vector<__half> f((size_t)64 * Ls * Lh), b((size_t)64 * Ls * Lh);
+  for (int ah = 0; ah < Lh; ah++) for (int m = 0; m < 4; m++) for (int s = 0; s < Ls; s++) for (int n = 0; n < 4; n++) {
+    const double tr = Tc(ah, m, s, n, 0), ti = Tc(ah, m, s, n, 1);
+    // forward: row (ah, sp, hi, ri') with m = 2*hi + sp (fp16 fragment order), column (s, n, ri)
+    const int rowf = ah * 8 + ((m & 1) * 2 + (m >> 1)) * 2, colf = s * 8 + n * 2;
+    put(f, Ls, rowf, colf, tr); put(f, Ls, rowf, colf + 1, -ti); put(f, Ls, rowf + 1, colf, ti); put(f, Ls, rowf + 1, colf + 1, tr);
+    // backward (conj T): row (s, n, ri'), column (ah, m, ri)
+    const int rowb = s * 8 + n * 2, colb = ah * 8 + m * 2;
+    put(b, Lh, rowb, colb, tr); put(b, Lh, rowb, colb + 1, ti); put(b, Lh, rowb + 1, colb, -ti); put(b, Lh, rowb + 1, colb + 1, tr);
+  }
+  CUDA_OK(ctx, up(ctx->Bfwd, f, st)); CUDA_OK(ctx, up(ctx->Bbwd, b, st)); CUDA_OK(ctx, cudaStreamSynchronize(st));
+  return MSPCG_OK;
+}
+
 int check_ready(mspcg_ctx* c, bool need_gauge) {
   if (!c) return MSPCG_EINVAL;
   if (!c->have_ws) return fail(c, MSPCG_ENOWORKSPACE, "mspcg_set_workspace has not been called");
@@ -642,6 +664,89 @@ int solve_impl(mspcg_ctx* c, const double* b_abi, double* x_abi, const mspcg_sol
 
 }  // namespace
 
+// ------------------------------------------------------------------------------------------- training of T (A12)
+// w = (+)_s A_s v on fp64 NATIVE vectors, through the block operator in the inner precision T (double: in place).
+template <typename T>
+cudaError_t block_operator64(mspcg_ctx* c, const double* v, double* w, cudaStream_t st) {
+  const Geometry& g = c->lat.blk;
+  OpView<T> view = make_view<T>(c, c->blkI, g, c->gblk, c->Ls, false);
+  c->cur_geom = 1;
+  const long Vh = c->lat.V4 / 2;
+  cudaError_t e;
+  if (sizeof(T) == 8) {
+    DISPATCH_LS(c->Ls, return (apply_normal<T, LS>(c, view, mphi_plain<T>((const T*)v), (const T*)v, (T*)w, nullptr, st)));
+  }
+  if ((e = convert_any(c, v, 8, c->in_p, (int)sizeof(T), Vh, c->Ls, st)) != cudaSuccess) return e;
+  DISPATCH_LS(c->Ls, e = (apply_normal<T, LS>(c, view, mphi_plain<T>((const T*)c->in_p), (const T*)c->in_p, (T*)c->in_q, nullptr, st)));
+  if (e != cudaSuccess) return e;
+  return convert_any(c, c->in_q, (int)sizeof(T), w, 8, Vh, c->Ls, st);
+}
+
+// chi2 = sum_i |M (T^dag Ahat T + mu) v_i - v_i|^2 and (optionally) G = d chi2 / d conj(T) = sum_i (c_i v_i^dag + a_i g_i^dag),
+// e = M w - v, g = M e, a = Ahat T v, c = Ahat T g (eq. 22; reading R20).
+template <typename T>
+int train_eval_impl(mspcg_ctx* c, const double* v_abi, int nvec, int k, double* chi2, double* grad_host, cudaStream_t st) {
+  typedef typename std::conditional<sizeof(T) == 8, double, float>::type TX;
+  const int Ls = c->Ls, Lh = c->Ls_hat;
+  const long Vh = c->lat.V4 / 2, nreal = v5h(c, Ls) * 24;
+  const size_t nG = (size_t)16 * Lh * Ls * 2;
+  double *V = (double*)c->stage_in, *W = (double*)c->stage_out, *E = c->v_t64, *Gv = c->v_rhi;
+  const int spb = 32;
+  const unsigned oblocks = (unsigned)((Vh + spb - 1) / spb);
+  const size_t osm = sizeof(double) * 24 * (Ls + Lh);
+  SOLVE_CUDA(cudaMemsetAsync(c->Gdev, 0, sizeof(double) * nG, st));
+  SOLVE_CUDA(sc_zero(c, 2, st));
+  for (int i = 0; i < nvec; i++) {
+    SOLVE_CUDA(pack_any(c, v_abi + (size_t)i * nreal, V, MSPCG_F64, 1, st));
+    SOLVE_CUDA(precond_dispatch<double>(c, V, W, k, true, st));                       // W = (T^dag Ahat T + mu) V ; in_x = a
+    SOLVE_CUDA(block_operator64<T>(c, W, E, st));
+    SOLVE_CUDA(axpby<double>(c, -1.0, V, 1.0, E, nreal, st));                          // e = M w - v
+    SOLVE_CUDA(dot2<double>(c, E, E, nullptr, nreal, st));                             // chi2 += |e|^2 (accumulates in sc[0])
+    if (grad_host) {
+      SOLVE_CUDA(block_operator64<T>(c, E, Gv, st));                                   // g = M e
+      k_outer_T<TX><<<oblocks, 512, osm, st>>>((const TX*)c->in_x, Gv, Vh, Ls, Lh, spb, c->Gdev); c->launches++;
+      SOLVE_CUDA(precond_dispatch<double>(c, Gv, W, k, true, st));                     // in_x = c = Ahat T g
+      k_outer_T<TX><<<oblocks, 512, osm, st>>>((const TX*)c->in_x, V, Vh, Ls, Lh, spb, c->Gdev); c->launches++;
+      SOLVE_CUDA(cudaPeekAtLastError());
+    }
+  }
+  SOLVE_CUDA(sc_read(c, 1, st));
+  *chi2 = c->sc_host[0];
+  if (grad_host) { SOLVE_CUDA(cudaMemcpyAsync(grad_host, c->Gdev, sizeof(double) * nG, cudaMemcpyDeviceToHost, st)); SOLVE_CUDA(cudaStreamSynchronize(st)); }
+  return MSPCG_OK;
+}
+
+// Real stationary point with the smallest value of the quartic through five equally spaced points (exact line search
+// when Ahat is linear): Lagrange fit by elimination, cubic derivative solved in closed form.
+double quartic_argmin(const double eta[5], const double val[5]) {
+  double A[5][6];
+  const double sc = eta[4] != 0 ? eta[4] : 1.0;   // work in x = eta / eta_max
+  for (int i = 0; i < 5; i++) { double x = eta[i] / sc, p = 1; for (int j = 0; j < 5; j++) { A[i][j] = p; p *= x; } A[i][5] = val[i]; }
+  for (int col = 0; col < 5; col++) {
+    int piv = col; for (int r = col + 1; r < 5; r++) if (std::fabs(A[r][col]) > std::fabs(A[piv][col])) piv = r;
+    for (int j = 0; j < 6; j++) std::swap(A[col][j], A[piv][j]);
+    for (int r = 0; r < 5; r++) if (r != col) { double f = A[r][col] / A[col][col]; for (int j = col; j < 6; j++) A[r][j] -= f * A[col][j]; }
+  }
+  double cf[5]; for (int i = 0; i < 5; i++) cf[i] = A[i][5] / A[i][i];           // val = sum cf[j] x^j
+  auto P = [&](double x) { return (((cf[4] * x + cf[3]) * x + cf[2]) * x + cf[1]) * x + cf[0]; };
+  // derivative 4 c4 x^3 + 3 c3 x^2 + 2 c2 x + c1 = 0
+  double a3 = 4 * cf[4], a2 = 3 * cf[3], a1 = 2 * cf[2], a0 = cf[1];
+  double roots[3]; int nr = 0;
+  if (std::fabs(a3) < 1e-300) {
+    if (std::fabs(a2) > 1e-300) { double disc = a1 * a1 - 4 * a2 * a0; if (disc >= 0) { roots[nr++] = (-a1 + std::sqrt(disc)) / (2 * a2); roots[nr++] = (-a1 - std::sqrt(disc)) / (2 * a2); } }
+    else if (std::fabs(a1) > 1e-300) roots[nr++] = -a0 / a1;
+  } else {
+    double b = a2 / a3, cc = a1 / a3, d = a0 / a3;
+    double p = cc - b * b / 3, q = 2 * b * b * b / 27 - b * cc / 3 + d, disc = q * q / 4 + p * p * p / 27;
+    if (disc > 0) { double sq = std::sqrt(disc); roots[nr++] = std::cbrt(-q / 2 + sq) + std::cbrt(-q / 2 - sq) - b / 3; }
+    else { double r = std::sqrt(-p * p * p / 27), phi = std::acos(std::fmax(-1.0, std::fmin(1.0, -q / (2 * (r > 0 ? r : 1e-300))))), m = 2 * std::sqrt(-p / 3);
+      for (int j = 0; j < 3; j++) roots[nr++] = m * std::cos((phi + 2 * M_PI * j) / 3) - b / 3; }
+  }
+  if (nr == 0) { int best = 0; for (int i = 1; i < 5; i++) if (val[i] < val[best]) best = i; return eta[best]; }
+  double bx = roots[0]; for (int j = 1; j < nr; j++) if (P(roots[j]) < P(bx)) bx = roots[j];
+  return bx * sc;
+}
+
 // ================================================================================================== C ABI
 extern "C" {
 
@@ -729,23 +834,7 @@ int mspcg_set_workspace(mspcg_ctx* ctx, void* workspace_dev, size_t bytes, void*
   if (ctx->Ls_hat) {
     CUDA_OK(ctx, upload_mats<double>(ctx->md_hat, ctx->hm_hat, st)); CUDA_OK(ctx, upload_mats<float>(ctx->mf32_hat, ctx->hm_hat, st));
     CUDA_OK(ctx, upload_frags(ctx->mfr_hat, ctx->hm_hat, ctx->Ls_hat, st));
-    CUDA_OK(ctx, up(ctx->Tm, ctx->T_host, st)); CUDA_OK(ctx, cudaStreamSynchronize(st));
-    { // B-operand images (UMMA canonical K-major, no swizzle: element (n, k) at (n/8)*KG*64 + (k/8)*64 + (n%8)*8 + k%8 halves)
-      const int Ls = ctx->Ls, Lh = ctx->Ls_hat;
-      auto Tc = [&](int ah, int m, int s, int n, int ri) { return ctx->T_host[((((size_t)ah * 4 + m) * (4 * Ls)) + s * 4 + n) * 2 + ri]; };
-      auto put = [&](std::vector<__half>& img, int KG, int n, int k, double v) { img[(size_t)(n / 8) * KG * 64 + (size_t)(k / 8) * 64 + (n % 8) * 8 + (k % 8)] = __float2half_rn((float)v); };
-      std::vector<__half> f((size_t)64 * Ls * Lh), b((size_t)64 * Ls * Lh);
-      for (int ah = 0; ah < Lh; ah++) for (int m = 0; m < 4; m++) for (int s = 0; s < Ls; s++) for (int n = 0; n < 4; n++) {
-        const double tr = Tc(ah, m, s, n, 0), ti = Tc(ah, m, s, n, 1);
-        // forward: row (ah, sp, hi, ri') with m = 2*hi + sp (fp16 fragment order), column (s, n, ri)
-        const int rowf = ah * 8 + ((m & 1) * 2 + (m >> 1)) * 2, colf = s * 8 + n * 2;
-        put(f, Ls, rowf, colf, tr); put(f, Ls, rowf, colf + 1, -ti); put(f, Ls, rowf + 1, colf, ti); put(f, Ls, rowf + 1, colf + 1, tr);
-        // backward (conj T): row (s, n, ri'), column (ah, m, ri)
-        const int rowb = s * 8 + n * 2, colb = ah * 8 + m * 2;
-        put(b, Lh, rowb, colb, tr); put(b, Lh, rowb, colb + 1, ti); put(b, Lh, rowb + 1, colb, -ti); put(b, Lh, rowb + 1, colb + 1, tr);
-      }
-      CUDA_OK(ctx, up(ctx->Bfwd, f, st)); CUDA_OK(ctx, up(ctx->Bbwd, b, st)); CUDA_OK(ctx, cudaStreamSynchronize(st));
-    }
+    { int rc_ = upload_T(ctx, st); if (rc_) return rc_; }
   }
   if (!ctx->sc_host) CUDA_OK(ctx, cudaMallocHost(&ctx->sc_host, sizeof(double) * 16));
   { int dev = 0, n = 0;
@@ -859,6 +948,55 @@ int mspcg_solve(mspcg_ctx* ctx, const double* b_dev, double* x_dev, const mspcg_
   if (params->sloppy_prec == MSPCG_F64) return solve_impl<double>(ctx, b_dev, x_dev, params, stats, st);
   if (params->sloppy_prec == MSPCG_F32) return solve_impl<float>(ctx, b_dev, x_dev, params, stats, st);
   return solve_impl<__half>(ctx, b_dev, x_dev, params, stats, st);
+}
+
+int mspcg_update_T(mspcg_ctx* ctx, const double* T_host, double mu, void* stream) {
+  int rc = check_ready(ctx, false); if (rc) return rc;
+  if (!ctx->Ls_hat || !T_host) return fail(ctx, MSPCG_EINVAL, "mspcg_update_T needs mspcg_set_reduced_ls before the workspace was sized");
+  ctx->T_host.assign(T_host, T_host + (size_t)4 * ctx->Ls_hat * 4 * ctx->Ls * 2);
+  ctx->mu_shift = mu;
+  return upload_T(ctx, (cudaStream_t)stream);
+}
+
+int mspcg_train_eval(mspcg_ctx* ctx, const double* v_dev, int nvec, int n_inner, double* chi2_host, double* grad_host, void* stream) {
+  int rc = check_ready(ctx, true); if (rc) return rc;
+  if (!ctx->Ls_hat || !v_dev || nvec < 1 || !chi2_host || n_inner < 1 || n_inner > KMAX) return fail(ctx, MSPCG_EINVAL, "bad argument or no reduced-Ls set-up");
+  if (ctx->inner_prec == MSPCG_F16) return fail(ctx, MSPCG_EINVAL, "training runs with inner_prec fp64 or fp32 (train there, use T anywhere)");
+  mspcg_ctx* c = ctx;
+  if (ctx->inner_prec == MSPCG_F64) return train_eval_impl<double>(c, v_dev, nvec, n_inner, chi2_host, grad_host, (cudaStream_t)stream);
+  return train_eval_impl<float>(c, v_dev, nvec, n_inner, chi2_host, grad_host, (cudaStream_t)stream);
+}
+
+int mspcg_train_T(mspcg_ctx* ctx, const double* v_dev, int nvec, int n_inner, int n_steps, double momentum, double* T_host_out,
+                  double* chi2_history_host, void* stream) {
+  int rc = check_ready(ctx, true); if (rc) return rc;
+  if (!ctx->Ls_hat || n_steps < 0 || !T_host_out) return fail(ctx, MSPCG_EINVAL, "bad argument or no reduced-Ls set-up");
+  const size_t n = (size_t)16 * ctx->Ls_hat * ctx->Ls * 2;
+  std::vector<double> T(ctx->T_host), G(n), P(n, 0.0), Tt(n);
+  const double mu = ctx->mu_shift;
+  double val = 0;
+  for (int step = 0; step < n_steps; step++) {
+    if ((rc = mspcg_train_eval(ctx, v_dev, nvec, n_inner, &val, G.data(), stream))) return rc;
+    if (chi2_history_host) chi2_history_host[step] = val;
+    double g2 = 0; for (size_t i = 0; i < n; i++) g2 += G[i] * G[i];
+    if (!(g2 > 0)) break;
+    for (size_t i = 0; i < n; i++) P[i] = -G[i] + momentum * P[i];                // momentum method ([25])
+    const double eta0 = val / g2;
+    const double eta[5] = {0.0, 0.5 * eta0, eta0, 1.5 * eta0, 2.0 * eta0};
+    double vals[5] = {val, 0, 0, 0, 0};
+    for (int j = 1; j < 5; j++) {
+      for (size_t i = 0; i < n; i++) Tt[i] = T[i] + eta[j] * P[i];
+      if ((rc = mspcg_update_T(ctx, Tt.data(), mu, stream))) return rc;
+      if ((rc = mspcg_train_eval(ctx, v_dev, nvec, n_inner, &vals[j], nullptr, stream))) return rc;
+    }
+    const double es = quartic_argmin(eta, vals);
+    for (size_t i = 0; i < n; i++) T[i] += es * P[i];
+    if ((rc = mspcg_update_T(ctx, T.data(), mu, stream))) return rc;
+  }
+  if ((rc = mspcg_train_eval(ctx, v_dev, nvec, n_inner, &val, nullptr, stream))) return rc;
+  if (chi2_history_host) chi2_history_host[n_steps] = val;
+  memcpy(T_host_out, T.data(), n * sizeof(double));
+  return MSPCG_OK;
 }
 
 long mspcg_launch_count(const mspcg_ctx* ctx) { return ctx ? ctx->launches : 0; }
