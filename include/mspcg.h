@@ -118,7 +118,9 @@ int mspcg_update_T(mspcg_ctx* ctx, const double* T_host, double mu, void* stream
  * one context, use T in any).  Synchronous. */
 int mspcg_train_eval(mspcg_ctx* ctx, const double* v_dev, int nvec, int n_inner, double* chi2_host, double* grad_host, void* stream);
 /* n_steps of: P = -grad + momentum * P_prev; chi2 at eta0 * (0, 1/2, 1, 3/2, 2), eta0 = chi2 / |grad|^2; T += eta* P with eta*
- * the minimiser of the quartic through the five values ("line search", "momentum method").  The context's T
+ * the minimiser over [0, 2 eta0] of the quartic through the five values ("line search", "momentum method"), kept
+ * only if the loss there is not above the best sampled value; a step without decrease drops the momentum and quarters eta0.
+ * The context's T
  * is updated; T_host_out (HOST, layout of T_host) receives it; chi2_history_host (HOST, n_steps + 1 doubles or NULL) the
  * loss before every step and after the last. */
 int mspcg_train_T(mspcg_ctx* ctx, const double* v_dev, int nvec, int n_inner, int n_steps, double momentum, double* T_host_out,

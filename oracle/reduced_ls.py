@@ -106,24 +106,43 @@ def chi2_and_gradient(M_apply, Ahat_apply, T, mu, vs):
 
 
 def quartic_minimum(etas, vals):
-    """chi2(T + eta P) is a quartic in eta when Ahat is linear: fit it through five evaluations and return the real
-    stationary point with the smallest fitted value ("line search")."""
-    coef = np.polyfit(np.asarray(etas, dtype=np.float64), np.asarray(vals, dtype=np.float64), 4)
+    """chi2(T + eta P) is a quartic in eta when Ahat is linear: fit it through five evaluations and return the minimiser
+    of the fit over the sampled interval [etas[0], etas[-1]] ("line search"): the candidates are the real
+    stationary points inside the interval and the sample points themselves.  (The fixed-count CG is only approximately
+    linear, so the fit is not trusted outside the interval it was measured on.)"""
+    etas = np.asarray(etas, dtype=np.float64)
+    coef = np.polyfit(etas / etas[-1], np.asarray(vals, dtype=np.float64), 4)
     roots = np.roots(np.polyder(coef))
-    cand = [r.real for r in roots if abs(r.imag) <= 1e-9 * max(1.0, abs(r.real))]
-    if not cand:
-        return float(etas[int(np.argmin(vals))])
-    return float(min(cand, key=lambda x: np.polyval(coef, x)))
+    cand = [float(x) for x in etas / etas[-1]]
+    cand += [r.real for r in roots if abs(r.imag) <= 1e-9 * max(1.0, abs(r.real)) and 0.0 <= r.real <= 1.0]
+    return float(min(cand, key=lambda x: np.polyval(coef, x))) * float(etas[-1])
 
 
-def train_step(M_apply, Ahat_apply, T, mu, vs, direction_prev=None, momentum=0.0, eta0=None):
+def train_step(M_apply, Ahat_apply, T, mu, vs, direction_prev=None, momentum=0.0, scale=1.0):
     """One step: P = -G + momentum * P_prev; five evaluations at eta0 * (0, 1/2, 1, 3/2, 2); T <- T + eta* P.
-    eta0 defaults to chi2 / |G|^2 (the Newton-like scale of a quadratic).  Returns (T_new, P, chi2_before, eta*)."""
+    eta0 = scale * chi2 / |G|^2 (the Newton-like scale of a quadratic).  Returns (T_new, P, chi2_before, eta*)."""
     val, G = chi2_and_gradient(M_apply, Ahat_apply, T, mu, vs)
     P = -G if direction_prev is None else -G + momentum * direction_prev
-    if eta0 is None:
-        eta0 = val / float(np.vdot(G, G).real)
+    eta0 = scale * val / float(np.vdot(G, G).real)
     etas = [0.0, 0.5 * eta0, eta0, 1.5 * eta0, 2.0 * eta0]
     vals = [val] + [chi2(M_apply, Ahat_apply, T + h * P, mu, vs) for h in etas[1:]]
     eta = quartic_minimum(etas, vals)
+    best = int(np.argmin(vals))
+    if eta not in etas and chi2(M_apply, Ahat_apply, T + eta * P, mu, vs) > vals[best]:
+        eta = etas[best]          # the fit promised more than the loss delivers: keep the best measured point
     return T + eta * P, P, val, eta
+
+
+def train(M_apply, Ahat_apply, T, mu, vs, n_steps, momentum):
+    """n_steps of train_step.  When a step finds no decrease (eta* = 0) the momentum is dropped and the step scale is
+    quartered; after a successful step the scale doubles back towards 1.  Returns (T, [chi2 before each step, final chi2])."""
+    P, scale, hist = None, 1.0, []
+    for _ in range(n_steps):
+        T, P, val, eta = train_step(M_apply, Ahat_apply, T, mu, vs, P, momentum, scale)
+        hist.append(val)
+        if eta == 0.0:
+            P, scale = None, scale * 0.25
+        else:
+            scale = min(1.0, scale * 2.0)
+    hist.append(chi2(M_apply, Ahat_apply, T, mu, vs))
+    return T, hist

@@ -4,6 +4,7 @@
 // kernels.cuh; this file only sequences launches and moves scalars.  There is no CPU fallback.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -716,8 +717,9 @@ int train_eval_impl(mspcg_ctx* c, const double* v_abi, int nvec, int k, double* 
   return MSPCG_OK;
 }
 
-// Real stationary point with the smallest value of the quartic through five equally spaced points (exact line search
-// when Ahat is linear): Lagrange fit by elimination, cubic derivative solved in closed form.
+// Minimiser over the sampled interval of the quartic through five equally spaced points (exact line search when Ahat is
+// linear; not trusted outside the interval because the fixed-count CG is only approximately linear):
+// fit by elimination, cubic derivative solved in closed form.
 double quartic_argmin(const double eta[5], const double val[5]) {
   double A[5][6];
   const double sc = eta[4] != 0 ? eta[4] : 1.0;   // work in x = eta / eta_max
@@ -742,8 +744,10 @@ double quartic_argmin(const double eta[5], const double val[5]) {
     else { double r = std::sqrt(-p * p * p / 27), phi = std::acos(std::fmax(-1.0, std::fmin(1.0, -q / (2 * (r > 0 ? r : 1e-300))))), m = 2 * std::sqrt(-p / 3);
       for (int j = 0; j < 3; j++) roots[nr++] = m * std::cos((phi + 2 * M_PI * j) / 3) - b / 3; }
   }
-  if (nr == 0) { int best = 0; for (int i = 1; i < 5; i++) if (val[i] < val[best]) best = i; return eta[best]; }
-  double bx = roots[0]; for (int j = 1; j < nr; j++) if (P(roots[j]) < P(bx)) bx = roots[j];
+  // minimiser of the fit over the sampled interval: stationary points inside [0, 1] and the sample points themselves
+  double bx = 0.0, bv = P(0.0);
+  for (int i = 1; i < 5; i++) { const double x = eta[i] / sc; if (P(x) < bv) { bv = P(x); bx = x; } }
+  for (int j = 0; j < nr; j++) if (roots[j] >= 0.0 && roots[j] <= 1.0 && P(roots[j]) < bv) { bv = P(roots[j]); bx = roots[j]; }
   return bx * sc;
 }
 
@@ -974,14 +978,14 @@ int mspcg_train_T(mspcg_ctx* ctx, const double* v_dev, int nvec, int n_inner, in
   const size_t n = (size_t)16 * ctx->Ls_hat * ctx->Ls * 2;
   std::vector<double> T(ctx->T_host), G(n), P(n, 0.0), Tt(n);
   const double mu = ctx->mu_shift;
-  double val = 0;
+  double val = 0, scale = 1.0;
   for (int step = 0; step < n_steps; step++) {
     if ((rc = mspcg_train_eval(ctx, v_dev, nvec, n_inner, &val, G.data(), stream))) return rc;
     if (chi2_history_host) chi2_history_host[step] = val;
     double g2 = 0; for (size_t i = 0; i < n; i++) g2 += G[i] * G[i];
     if (!(g2 > 0)) break;
     for (size_t i = 0; i < n; i++) P[i] = -G[i] + momentum * P[i];                // momentum method ([25])
-    const double eta0 = val / g2;
+    const double eta0 = scale * val / g2;
     const double eta[5] = {0.0, 0.5 * eta0, eta0, 1.5 * eta0, 2.0 * eta0};
     double vals[5] = {val, 0, 0, 0, 0};
     for (int j = 1; j < 5; j++) {
@@ -989,8 +993,19 @@ int mspcg_train_T(mspcg_ctx* ctx, const double* v_dev, int nvec, int n_inner, in
       if ((rc = mspcg_update_T(ctx, Tt.data(), mu, stream))) return rc;
       if ((rc = mspcg_train_eval(ctx, v_dev, nvec, n_inner, &vals[j], nullptr, stream))) return rc;
     }
-    const double es = quartic_argmin(eta, vals);
+    double es = quartic_argmin(eta, vals);
+    int best = 0; for (int j = 1; j < 5; j++) if (vals[j] < vals[best]) best = j;
+    bool sampled = false; for (int j = 0; j < 5; j++) sampled = sampled || es == eta[j];
+    if (!sampled) {   // the fit promised more than the loss delivers: keep the best measured point
+      double ve = 0;
+      for (size_t i = 0; i < n; i++) Tt[i] = T[i] + es * P[i];
+      if ((rc = mspcg_update_T(ctx, Tt.data(), mu, stream))) return rc;
+      if ((rc = mspcg_train_eval(ctx, v_dev, nvec, n_inner, &ve, nullptr, stream))) return rc;
+      if (ve > vals[best]) es = eta[best];
+    }
     for (size_t i = 0; i < n; i++) T[i] += es * P[i];
+    if (es == 0.0) { std::fill(P.begin(), P.end(), 0.0); scale *= 0.25; }   // no decrease found: drop the momentum, shorten the step
+    else scale = std::fmin(1.0, scale * 2.0);
     if ((rc = mspcg_update_T(ctx, T.data(), mu, stream))) return rc;
   }
   if ((rc = mspcg_train_eval(ctx, v_dev, nvec, n_inner, &val, nullptr, stream))) return rc;

@@ -49,18 +49,14 @@ def test_loss_and_gradient_match_the_oracle():
     assert abs(val - val_o) <= 1e-9 * val_o
     assert rel(G, rl.T_to_abi(G_o)) <= 1e-8
     val2, _ = g.train_eval(dv, k, want_grad=False)
-    assert val2 == val
+    assert abs(val2 - val) <= 1e-12 * val      # atomics: summation order differs between runs
 
 
 def test_training_steps_follow_the_oracle_and_reduce_the_loss():
     dims, Ls, Lh, block, mu, k = (4, 2, 2, 4), 6, 4, (2, 2, 2, 2), 0.4, 4
     rl, M_apply, Ph, T, vs, dv, g = _setup(dims, Ls, Lh, block, mu)
     Ahat = lambda r: Ph(r, k)
-    To, P, hist_o = T, None, []
-    for _ in range(2):
-        To, P, v0, eta = rl.train_step(M_apply, Ahat, To, mu, vs, P, 0.5)
-        hist_o.append(v0)
-    hist_o.append(rl.chi2(M_apply, Ahat, To, mu, vs))
+    To, hist_o = rl.train(M_apply, Ahat, T, mu, vs, 2, 0.5)
     Tg, hist = g.train_T(dv, k, 2, momentum=0.5)
     assert np.all(np.diff(hist) < 0)
     assert rel(hist, hist_o) <= 1e-6
