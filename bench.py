@@ -342,18 +342,26 @@ def extras(torch, g, cfg, U, src, d_src, geo, peak, args):
     del x
     g.close()
     torch.cuda.empty_cache()
-    # reduced-Ls preconditioner with the UNTRAINED transfer matrix: cost per application and its
-    # effect on the outer iteration count (the trained T of eq. 22 is a set-up step)
-    Lh = cfg.get("Ls_hat", Ls // 2)
+    # reduced-Ls preconditioner: T trained with the library (eq. 22; set-up step, its time reported, not
+    # part of the solve) on residual vectors of a full-Ls MSPCG run, then MSPCG with z = T^dag CG_k[Mhat](T r) + mu r
+    from paper_2104_05615_b200.train_reduced_ls import train
+    Lh, mu = cfg.get("Ls_hat", Ls // 2), 0.3
+    t0 = time.time()
+    T, info = train(dims, Ls, dict(b=cfg["b"], c=cfg["c"], M5=cfg["M5"]), cfg["mf"], block, U, src, Lh, mu, k,
+                    n_vec=12, span=120, n_steps=args.train_steps, momentum=0.5)
+    torch.cuda.synchronize()
+    train_s = time.time() - t0
     gr = Mspcg(dims, Ls, cfg["b"], cfg["c"], cfg["M5"], cfg["mf"], block)
-    gr.set_reduced_ls(Lh, initial_T_abi(Ls, Lh), 0.5)
+    gr.set_reduced_ls(Lh, T, mu)
     gr.configure(F32, F16, 18)
     gr.load_gauge(U, -1)
     v, o = gr.pack(d_src, F32), gr.new_native(F32)
     ms = timed(torch, lambda: gr.apply_precond(v, k, F32, LAYOUT_NATIVE, out=o, use_reduced=1), steps, warm) / steps
     x, s = gr.solve(d_src, tol=1e-10, max_iter=200000, use_precond=True, n_inner=k, sloppy_prec=F32, delta=0.1, use_reduced_ls=True)
-    ex["reducedLs%d_untrainedT_mu0.5" % Lh] = dict(Mpre_ms=ms, solve=dict(seconds=s["seconds"], outer_iters=s["iters"], reliable_updates=s["reliable_updates"],
-                                                   inner_applies=s["inner_applies"], true_res=s["true_res"], rc=s["rc"]))
+    ex["reducedLs%d_trainedT_mu%.1f" % (Lh, mu)] = dict(
+        Mpre_ms=ms, train_seconds=train_s, train_steps=args.train_steps, chi2_first=float(info["chi2"][0]), chi2_last=float(info["chi2"][-1]),
+        solve=dict(seconds=s["seconds"], outer_iters=s["iters"], reliable_updates=s["reliable_updates"],
+                   inner_applies=s["inner_applies"], true_res=s["true_res"], rc=s["rc"]))
     del x, v, o
     gr.close()
     torch.cuda.empty_cache()
@@ -435,6 +443,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C2", choices=sorted(synth.CONFIGS))
     ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--train-steps", type=int, default=40, help="line-search steps of the T training in the extras")
     ap.add_argument("--reduced", type=int, default=0, help="profiling aid: run the step with the reduced-Ls preconditioner at this Ls_hat")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
