@@ -371,6 +371,19 @@ def extras(torch, g, cfg, U, src, d_src, geo, peak, args):
     ex["DdagD_fp16"] = time_op(g2, F16, 2)
     ex["Mpre_k%d_fp64" % k] = time_pre(g2, F64, 8, 8)
     g2.close()
+    torch.cuda.empty_cache()
+    # the same solves with an fp16 sloppy outer iteration (vectors rescaled at every residual replacement)
+    g3 = Mspcg(dims, Ls, cfg["b"], cfg["c"], cfg["M5"], cfg["mf"], block)
+    g3.configure(F16, F16, 18)
+    g3.load_gauge(U, -1)
+    sol = {}
+    for name, pre in (("CG", False), ("MSPCG", True)):
+        x, s = g3.solve(d_src, tol=1e-10, max_iter=200000, use_precond=pre, n_inner=k, sloppy_prec=F16, delta=0.1)
+        sol[name] = dict(seconds=s["seconds"], outer_iters=s["iters"], reliable_updates=s["reliable_updates"],
+                         inner_applies=s["inner_applies"], true_res=s["true_res"], rc=s["rc"])
+    ex["solve_tol1e-10_fp16outer_fp16inner"] = sol
+    del x
+    g3.close()
     return ex
 
 

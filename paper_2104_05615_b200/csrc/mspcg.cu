@@ -311,8 +311,8 @@ cudaError_t convert(mspcg_ctx* c, const void* a, void* b, long n_sites, int Ls, 
   c->launches++;
   return cudaPeekAtLastError();
 }
-cudaError_t convert_any(mspcg_ctx* c, const void* a, int pa, void* b, int pb, long n_sites, int Ls, cudaStream_t st) {
-#define CV(PA, TA, PB, TB) if (pa == PA && pb == PB) return convert<TA, TB>(c, a, b, n_sites, Ls, 1, nullptr, 0, 1.0, st);
+cudaError_t convert_any(mspcg_ctx* c, const void* a, int pa, void* b, int pb, long n_sites, int Ls, cudaStream_t st, double factor = 1.0) {
+#define CV(PA, TA, PB, TB) if (pa == PA && pb == PB) return convert<TA, TB>(c, a, b, n_sites, Ls, 1, nullptr, 0, factor, st);
   CV(8, double, 8, double) CV(8, double, 4, float) CV(8, double, 2, __half)
   CV(4, float, 8, double) CV(4, float, 4, float) CV(4, float, 2, __half)
   CV(2, __half, 8, double) CV(2, __half, 4, float) CV(2, __half, 2, __half)
@@ -592,7 +592,12 @@ int solve_impl(mspcg_ctx* c, const double* b_abi, double* x_abi, const mspcg_sol
   } else {
     double rnorm = 0, maxr, rz = 0, alpha = 0, beta = 0;
     SOLVE_CUDA(true_residual(&rnorm));                       // r0 = b - A x0 (R15)
-    SOLVE_CUDA(convert_any(c, rhi, 8, rlo, sp, Vh, Ls, st));
+    // fp16 sloppy vectors are kept in units of sigma ~ |r| at the last residual replacement (r_lo = r_hi / sigma, so
+    // x_lo = x_true / sigma, p likewise): alpha and beta are scale invariant, and fp16 never underflows as r shrinks.
+    const bool rescale = sizeof(TS) == 2;
+    const double unit = 16.0 / std::sqrt((double)nreal);   // |r_lo| = sqrt(n)/16: rms element 2^-4, three decades above the fp16 normal minimum
+    double sigma = (rescale && rnorm > 0) ? rnorm * unit : 1.0;
+    SOLVE_CUDA(convert_any(c, rhi, 8, rlo, sp, Vh, Ls, st, 1.0 / sigma));
     SOLVE_CUDA(cudaMemsetAsync(xlo, 0, sizeof(TS) * nreal, st));
     maxr = rnorm;
     if (rnorm <= prm->tol * bnorm) stt->converged = 1;
@@ -619,7 +624,7 @@ int solve_impl(mspcg_ctx* c, const double* b_abi, double* x_abi, const mspcg_sol
         k_outer_update<TS><<<(unsigned)((nchunk + 255) / 256), 256, 0, st>>>(p, Ap, rlo, xlo, nchunk, alpha, c->sc + 1);
         c->launches++; }
       SOLVE_CUDA(sc_read(c, 2, st));
-      rnorm = std::sqrt(c->sc_host[1]);
+      rnorm = std::sqrt(c->sc_host[1]) * sigma;
       k++;
       if (prm->history && k <= prm->history_len) prm->history[k - 1] = rnorm / bnorm;
       if (!(rnorm == rnorm)) { stt->breakdown = 1; rc = MSPCG_EBREAKDOWN; break; }
@@ -627,10 +632,15 @@ int solve_impl(mspcg_ctx* c, const double* b_abi, double* x_abi, const mspcg_sol
       if (rnorm <= prm->tol * bnorm || (sloppy && rnorm < prm->delta * maxr)) {
         // R17 residual replacement / R15 confirmation with the true residual
         SOLVE_CUDA(convert_any(c, xlo, sp, t64, 8, Vh, Ls, st));
-        SOLVE_CUDA(axpby<double>(c, 1.0, t64, 1.0, xhi, nreal, st));
+        SOLVE_CUDA(axpby<double>(c, sigma, t64, 1.0, xhi, nreal, st));
         SOLVE_CUDA(cudaMemsetAsync(xlo, 0, sizeof(TS) * nreal, st));
         SOLVE_CUDA(true_residual(&rnorm));
-        SOLVE_CUDA(convert_any(c, rhi, 8, rlo, sp, Vh, Ls, st));
+        if (rescale && rnorm > 0) {   // new unit: p keeps its true size, <z,r> follows
+          const double f = sigma / (rnorm * unit);
+          SOLVE_CUDA(axpby<TS>(c, 0.0, p, f, p, nreal, st));
+          rz *= f * f; sigma = rnorm * unit;
+        }
+        SOLVE_CUDA(convert_any(c, rhi, 8, rlo, sp, Vh, Ls, st, 1.0 / sigma));
         maxr = rnorm; stt->reliable_updates++; replaced = true;
         if (rnorm <= prm->tol * bnorm) { stt->converged = 1; break; }
       }
@@ -644,9 +654,9 @@ int solve_impl(mspcg_ctx* c, const double* b_abi, double* x_abi, const mspcg_sol
       rz = rz_new;
     }
     if (!stt->converged && rc == MSPCG_OK) rc = MSPCG_ENOCONV;
-    // x = x_hi + x_lo, true residual, unpack
+    // x = x_hi + sigma x_lo, true residual, unpack
     SOLVE_CUDA(convert_any(c, xlo, sp, t64, 8, Vh, Ls, st));
-    SOLVE_CUDA(axpby<double>(c, 1.0, t64, 1.0, xhi, nreal, st));
+    SOLVE_CUDA(axpby<double>(c, sigma, t64, 1.0, xhi, nreal, st));
     double rn = 0;
     SOLVE_CUDA(true_residual(&rn));
     stt->outer_applies--;   // the closing residual check is bookkeeping, not part of the iteration

@@ -274,3 +274,18 @@ def test_reduced_ls_transfer_on_tcgen05_matches_generic_kernels(dims, Ls, Lh, bl
     for k in out:
         assert rel(out[k], ref) <= 2e-2
     assert rel(out["1"], out["0"]) <= 5e-3 and rel(out["1f32"], out["0f32"]) <= 5e-3
+
+
+def test_solve_fp16_sloppy_outer_iteration():
+    """fp16 storage of the outer iteration's r, x, p (BASELINE.json configs[4]: "outer fp32/fp16 with fp64 reliable updates"):
+    the vectors are rescaled at every residual replacement, so fp16 never underflows on the way to 1e-10."""
+    dims, Ls, block = (4, 4, 4, 8), 8, (2, 2, 2, 4)
+    ora, g, torch = setup(dims, Ls, 0.01, block, eps=0.3, outer=F16, inner=F16)
+    b = synth.gaussian_spinor_abi(dims, Ls, 17)
+    x_ora, _ = ora.solve(b, tol=1e-11, use_precond=False)
+    for scale in (1.0, 1e-12):     # a tiny right-hand side must not matter
+        db = dev(torch, b * scale)
+        for pre in (False, True):
+            x, s = g.solve(db, tol=1e-10, use_precond=pre, n_inner=5, sloppy_prec=F16, delta=0.1)
+            assert s["rc"] == 0 and s["true_res"] <= 1e-10 and s["reliable_updates"] >= 5
+            assert rel(x.cpu().numpy() / scale, x_ora) <= 1e-8
