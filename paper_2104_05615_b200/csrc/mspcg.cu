@@ -137,15 +137,23 @@ template <typename C> void carve_mats(Arena& a, MatSet<C>& m, int Ls) {
 void carve_frags(Arena& a, MatFrag& m) {
   m.K2 = a.take<uint4>(64); m.K3a = a.take<uint4>(64); m.K3b = a.take<uint4>(64); m.K4 = a.take<uint4>(64); m.K5 = a.take<uint4>(64);
 }
-void carve_op(Arena& a, OpBuf& o, const Geometry& g, int prec, int ng, int Ls) {
+void carve_links(Arena& a, OpBuf& o, const Geometry& g, int prec, int ng) {
   o.prec = prec; o.ng = ng; o.have = true;
   size_t nblk = g.nblk;
   o.linksE = a.take_bytes(nblk * g.nE * 8 * ng * prec); o.linksO = a.take_bytes(nblk * g.nO * 8 * ng * prec);
   o.flipE = a.take<uint8_t>(nblk * g.nE); o.flipO = a.take<uint8_t>(nblk * g.nO);
-  size_t site = (size_t)Ls * 24 * prec;
+}
+void carve_temps(Arena& a, OpBuf& o, const Geometry& g, int Ls) {   // stage vectors of eq. 16: live only inside one operator application
+  size_t nblk = g.nblk, site = (size_t)Ls * 24 * o.prec;
   o.t1 = a.take_bytes(nblk * g.nE0 * site); o.tO = a.take_bytes(nblk * g.nO * site);
   o.y = a.take_bytes(nblk * g.nE0 * site); o.w = a.take_bytes(nblk * g.nE * site);
 }
+// Workspace layout.  Memory is sized for 180 GB at the largest configuration (48^3 x 96, Ls 12): buffers that are never live
+// at the same time share storage --
+//   * the stage vectors of the fp64 operator (used by residual replacements and fp64 applies) overlay the stage vectors of
+//     the sloppy operator, of the block operator and the inner-CG vectors (none holds data between two calls);
+//   * the staging buffers of the ABI-layout and *_host entry points overlay the solver's fp64 vectors (a solve and an apply
+//     call never run at the same time on one context).
 void carve(mspcg_ctx* c, Arena& a) {
   const Lattice& L = c->lat;
   carve_geom(a, c->gfull, L.full); carve_geom(a, c->gblk, L.blk);
@@ -155,19 +163,25 @@ void carve(mspcg_ctx* c, Arena& a) {
   c->rho = a.take<double>((size_t)(KMAX + 1) * L.nblk); c->pq = a.take<double>((size_t)KMAX * L.nblk);
   c->scale = a.take<float>(L.nblk); c->sc = a.take<double>(16);
   if (c->Ls_hat) { size_t nt = (size_t)4 * c->Ls_hat * 4 * c->Ls; c->Tm = a.take<double>(nt * 2); c->Bfwd = a.take<__half>(nt * 4); c->Bbwd = a.take<__half>(nt * 4); c->Gdev = a.take<double>(nt * 2); }
-  carve_op(a, c->full64, L.full, MSPCG_F64, 18, c->Ls);
-  if (c->outer_prec != MSPCG_F64) carve_op(a, c->fullS, L.full, c->outer_prec, c->recon, c->Ls);
-  carve_op(a, c->blkI, L.blk, c->inner_prec, c->inner_prec == MSPCG_F64 ? 18 : c->recon, c->Ls);
+  carve_links(a, c->full64, L.full, MSPCG_F64, 18);
+  if (c->outer_prec != MSPCG_F64) carve_links(a, c->fullS, L.full, c->outer_prec, c->recon);
+  carve_links(a, c->blkI, L.blk, c->inner_prec, c->inner_prec == MSPCG_F64 ? 18 : c->recon);
+  a.off = (a.off + 255) & ~(size_t)255;
+  Arena u1 = a, u2 = a;                                   // two overlays of the same region
+  carve_temps(u1, c->full64, L.full, c->Ls);
+  if (c->outer_prec != MSPCG_F64) carve_temps(u2, c->fullS, L.full, c->Ls);
+  carve_temps(u2, c->blkI, L.blk, c->Ls);
   size_t ni = vec_bytes(c, c->inner_prec, c->Ls);
-  c->in_r = a.take_bytes(ni); c->in_p = a.take_bytes(ni); c->in_q = a.take_bytes(ni);
-  c->in_x = a.take_bytes(vec_bytes(c, c->inner_prec == MSPCG_F64 ? MSPCG_F64 : MSPCG_F32, c->Ls));
+  c->in_r = u2.take_bytes(ni); c->in_p = u2.take_bytes(ni); c->in_q = u2.take_bytes(ni);
+  c->in_x = u2.take_bytes(vec_bytes(c, c->inner_prec == MSPCG_F64 ? MSPCG_F64 : MSPCG_F32, c->Ls));
+  a.off = u1.off > u2.off ? u1.off : u2.off;
   size_t n64 = vec_bytes(c, MSPCG_F64, c->Ls), nS = vec_bytes(c, c->outer_prec, c->Ls);
   c->v_b = (double*)a.take_bytes(n64); c->v_xhi = (double*)a.take_bytes(n64); c->v_rhi = (double*)a.take_bytes(n64);
   c->v_t64 = (double*)a.take_bytes(n64);
   c->v_xlo = a.take_bytes(nS); c->v_rlo = a.take_bytes(nS); c->v_p = a.take_bytes(nS); c->v_Ap = a.take_bytes(nS);
   c->v_z = a.take_bytes(nS);
-  c->stage_in = a.take_bytes(n64); c->stage_out = a.take_bytes(n64);
-  c->abi_in = (double*)a.take_bytes(n64); c->abi_out = (double*)a.take_bytes(n64);
+  c->stage_in = c->v_b; c->stage_out = c->v_xhi;
+  c->abi_in = c->v_rhi; c->abi_out = c->v_t64;
 }
 
 // ------------------------------------------------------------------------------------------------ per-launch timing
