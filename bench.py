@@ -195,17 +195,23 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
         barrier = dist.barrier
-    cfg = synth.CONFIGS[args.workload]
+    cfg = dict(synth.CONFIGS[args.workload])
+    if args.block:
+        cfg["block"] = tuple(int(x) for x in args.block.split(","))
     dims, Ls, block, k = cfg["dims"], cfg["Ls"], cfg["block"], cfg["n_inner"]
     U, src = make_inputs(cfg)
     g = Mspcg(dims, Ls, cfg["b"], cfg["c"], cfg["M5"], cfg["mf"], block)
     if args.reduced:   # profiling aid: the step's preconditioner becomes the reduced-Ls one (untrained T, eq. 20-21)
         g.set_reduced_ls(args.reduced, initial_T_abi(Ls, args.reduced), 0.5)
-    ws = g.configure(F32, F16, 18)
+    ws = g.configure(F32, F16, args.recon)
     g.load_gauge(U, -1)
     geo = g.geometry()
     d_src = torch.as_tensor(src.reshape(-1)).cuda()
     r32 = g.pack(d_src, F32)
+    big = ws > 100 * 2**30      # largest instance: no room for the fp64 ABI copies of the end-to-end leg
+    if big:
+        del d_src
+        torch.cuda.empty_cache()
     z32, q32 = g.new_native(F32), g.new_native(F32)
 
     def step():
@@ -213,10 +219,10 @@ def run_ours(args):
         g.apply_MdagM(r32, F32, LAYOUT_NATIVE, out=q32)
 
     # ---- work model of one step
-    fl_pre, by_pre = precond_work(geo, Ls, k, 2, 4, 18)
+    fl_pre, by_pre = precond_work(geo, Ls, k, 2, 4, args.recon)
     st_full = stage_sites(geo, True)
     fl_op = flops_normal(st_full, Ls)
-    by_op = sum(bytes_normal(st_full, Ls, 4, 18).values())
+    by_op = sum(bytes_normal(st_full, Ls, 4, args.recon).values())
     flops_step = fl_pre + fl_op
 
     # ---- the timed region (device-resident inputs)
@@ -234,22 +240,28 @@ def run_ours(args):
     value = world * flops_step / (ms_step * 1e-3) / 1e9
 
     # ---- end to end: same step through the *_host entry points, pinned host buffers, copies inside the timed region
-    h_in = torch.as_tensor(src.reshape(-1)).pin_memory()
-    h_z, h_q = torch.empty_like(h_in).pin_memory(), torch.empty_like(h_in).pin_memory()
+    if big:
+        ms_e2e = float("nan")
+    else:
+        h_in = torch.as_tensor(src.reshape(-1)).pin_memory()
+        h_z, h_q = torch.empty_like(h_in).pin_memory(), torch.empty_like(h_in).pin_memory()
 
-    def step_host():
-        g.apply_precond_host(h_in, h_z, k, F32)
-        g.apply_MdagM_host(h_in, h_q, F32)
+        def step_host():
+            g.apply_precond_host(h_in, h_z, k, F32)
+            g.apply_MdagM_host(h_in, h_q, F32)
 
-    e2e_steps = max(2, min(args.steps, 5))
-    ms_e2e = timed(torch, step_host, e2e_steps, 1, barrier) / e2e_steps
+        e2e_steps = max(2, min(args.steps, 5))
+        ms_e2e = timed(torch, step_host, e2e_steps, 1, barrier) / e2e_steps
     if world > 1:
         t = torch.tensor([ms_e2e], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms_e2e = float(t.item())
-    nb = h_in.numel() * 8
+    nb = src.size * 8
     e2e = dict(value=world * flops_step / (ms_e2e * 1e-3) / 1e9, unit=UNIT, ms_per_step=ms_e2e,
                h2d_bytes_per_step=2 * nb, d2h_bytes_per_step=2 * nb)
+    if big:
+        e2e = dict(value=None, unit=UNIT, skipped="workspace > 100 GiB: no device room for the fp64 ABI staging of the host leg",
+                   h2d_bytes_per_step=0, d2h_bytes_per_step=0)
 
     # ---- roofline of the dominant kernel: instrumented repetition of the same steps (CUDA events per launch)
     peak, peak_src = peaks()
@@ -259,8 +271,8 @@ def run_ours(args):
     tm = g.timing_read()
     g.timing(False)
     st_blk = stage_sites(geo, False)
-    bb = bytes_normal(st_blk, Ls, 2, 18, fused_pupdate=True, with_dot=True)
-    bf = bytes_normal(st_full, Ls, 4, 18)
+    bb = bytes_normal(st_blk, Ls, 2, args.recon, fused_pupdate=True, with_dot=True)
+    bf = bytes_normal(st_full, Ls, 4, args.recon)
     alg = {"blk.hop_k2k4": 0.5 * (bb["hop_k2"] + bb["hop_k4"]), "blk.hop_k3": bb["hop_k3"], "blk.hop_k5": bb["hop_k5"],
            "blk.mphi": bb["mphi"], "full.hop_k2k4": 0.5 * (bf["hop_k2"] + bf["hop_k4"]), "full.hop_k3": bf["hop_k3"],
            "full.hop_k5": bf["hop_k5"], "full.mphi": bf["mphi"]}
@@ -296,7 +308,7 @@ def run_ours(args):
                            flops_per_step=flops_step, alg_bytes_per_step=by_pre + by_op),
                gpu_launches=launches, clocks=clocks, e2e=e2e, roofline=roofline, kernels=kern,
                step_GBps_algorithmic=(by_pre + by_op) / (ms_step * 1e-3) / 1e9)
-    if rank == 0 and world == 1 and not args.no_extras:
+    if rank == 0 and world == 1 and not args.no_extras and not big:
         out["extras"] = extras(torch, g, cfg, U, src, d_src, geo, peak, args)
         out["cpu_baseline"] = cpu_baseline(cfg, U, src, geo)
     if rank == 0:
@@ -456,6 +468,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C2", choices=sorted(synth.CONFIGS))
     ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--block", default="", help="override the Dirichlet block, e.g. 12,12,12,12 (C5 block-size sweep)")
+    ap.add_argument("--recon", type=int, default=18, choices=[12, 18], help="link storage of the low-precision copies (12 = two rows, R8)")
     ap.add_argument("--train-steps", type=int, default=40, help="line-search steps of the T training in the extras")
     ap.add_argument("--reduced", type=int, default=0, help="profiling aid: run the step with the reduced-Ls preconditioner at this Ls_hat")
     args = ap.parse_args()
