@@ -182,6 +182,22 @@ def timed(torch, fn, steps, warmup, barrier=None):
     return e0.elapsed_time(e1)
 
 
+def max_over_ranks(ms, world, device):
+    """Replicas only: the only cross-rank step is the max of the device-timed region."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(flops_step, ms_step, world):
+    """Whole-job throughput of N independent replicas: N x (work of one replica) / (slowest replica's time)."""
+    return world * flops_step / (ms_step * 1e-3) / 1e9
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -232,12 +248,9 @@ def run_ours(args):
     ms = timed(torch, step, args.steps, args.warmup, barrier)
     launches = (g.launch_count() - n0) // (args.steps + args.warmup) * args.steps
     clocks = sampler.stop()
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, world, "cuda")
     ms_step = ms / args.steps
-    value = world * flops_step / (ms_step * 1e-3) / 1e9
+    value = aggregate_value(flops_step, ms_step, world)
 
     # ---- end to end: same step through the *_host entry points, pinned host buffers, copies inside the timed region
     if big:
@@ -252,10 +265,7 @@ def run_ours(args):
 
         e2e_steps = max(2, min(args.steps, 5))
         ms_e2e = timed(torch, step_host, e2e_steps, 1, barrier) / e2e_steps
-    if world > 1:
-        t = torch.tensor([ms_e2e], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
+    ms_e2e = max_over_ranks(ms_e2e, world, "cuda")
     nb = src.size * 8
     e2e = dict(value=world * flops_step / (ms_e2e * 1e-3) / 1e9, unit=UNIT, ms_per_step=ms_e2e,
                h2d_bytes_per_step=2 * nb, d2h_bytes_per_step=2 * nb)
