@@ -29,7 +29,7 @@ template <int LS> struct MmaCfg {
 };
 
 __device__ __forceinline__ void mma16816(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
-  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
+  asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
                : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
                : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
@@ -42,7 +42,7 @@ __device__ __forceinline__ void mma1688(float (&d)[4], uint32_t a0, uint32_t a1,
 }
 __device__ __forceinline__ uint32_t movmatrix_trans(uint32_t x) {
   uint32_t y;
-  asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;\n" : "=r"(y) : "r"(x));
+  asm("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;\n" : "=r"(y) : "r"(x));
   return y;
 }
 __device__ __forceinline__ uint32_t pack_h2(float lo, float hi) {
@@ -190,6 +190,12 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
                ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 
+__device__ __forceinline__ uint2 lds64(uint32_t addr) {
+  uint2 v;
+  asm volatile("ld.volatile.shared.v2.u32 {%0, %1}, [%2];\n" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+  return v;
+}
+
 template <int LS> struct MmaSmem {
   enum { SLOT = LS * 48, STAGE = 8 * SLOT, WARP = 2 * STAGE + 64, BLOCK = MmaCfg<LS>::NW * WARP };   // bytes
 };
@@ -300,13 +306,15 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
 #pragma unroll
     for (int m = 0; m < NMT; m++) { S[m][0] = S[m][1] = S[m][2] = S[m][3] = 0.f; }
     mbar_wait(bar_u32 + 8 * stg, parity);
-    const uint2* sb = reinterpret_cast<const uint2*>(wsm + stg * SM::STAGE);   // 64-bit reads: (hi0, hi1) of one sp
+    // 64-bit shared-memory reads ((hi0, hi1) of one sp).  ld.volatile keeps ptxas from merging the two halves of a chunk
+    // into one 128-bit read, so that the MMA's A operand {F.x, F.y, B.x, B.y} is allocated as one register quad without moves.
+    const uint32_t sb = stage_u32 + stg * SM::STAGE;
 #define MSPCG_HOP_MU(MU)                                                                       \
     if (have & (3u << (2 * MU))) {                                                             \
       uint2 Ff[NMT], Bb[NMT];                                                                  \
-      const uint2* pf = sb + (2 * MU) * (LS * 6); const uint2* pb = pf + LS * 6;               \
-      Ff[0] = pf[2 * fo0]; Ff[1] = pf[2 * fo0 + 1]; Bb[0] = pb[2 * fo0]; Bb[1] = pb[2 * fo0 + 1]; \
-      if (NSEG == 2) { Ff[NMT - 2] = pf[2 * fo1]; Ff[NMT - 1] = pf[2 * fo1 + 1]; Bb[NMT - 2] = pb[2 * fo1]; Bb[NMT - 1] = pb[2 * fo1 + 1]; } \
+      const uint32_t pf = sb + (2 * MU) * SM::SLOT, pb = pf + SM::SLOT;                        \
+      Ff[0] = lds64(pf + 16 * fo0); Bb[0] = lds64(pb + 16 * fo0); Ff[1] = lds64(pf + 16 * fo0 + 8); Bb[1] = lds64(pb + 16 * fo0 + 8); \
+      if (NSEG == 2) { Ff[NMT - 2] = lds64(pf + 16 * fo1); Bb[NMT - 2] = lds64(pb + 16 * fo1); Ff[NMT - 1] = lds64(pf + 16 * fo1 + 8); Bb[NMT - 1] = lds64(pb + 16 * fo1 + 8); } \
       hop_mu<MU, LS>(S, Ff, Bb, bfr[2 * MU], bfr[2 * MU + 1], sg);                             \
     }
     MSPCG_HOP_MU(0) MSPCG_HOP_MU(1) MSPCG_HOP_MU(2) MSPCG_HOP_MU(3)
