@@ -219,20 +219,27 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
   __shared__ double red[NW];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int g = lane >> 2, t = lane & 3;
-  const int blk = blockIdx.y;
+  int blk = blockIdx.y;
   const int stride = gridDim.x * NW;
   const float sg = (float)a.sg;
   float part = 0.f;
 
-  // per-block-row base pointers (64-bit once); everything below is 32-bit offsets in units of uint4
-  const uint4* in4 = reinterpret_cast<const uint4*>(a.in) + (long)blk * a.in_stride * (LS * 3);
-  uint4* out4 = reinterpret_cast<uint4*>(a.out) + (long)blk * a.out_stride * (LS * 3);
-  uint4* out24 = EPI == EPI_K3 ? reinterpret_cast<uint4*>(a.out2) + (long)blk * a.out2_stride * (LS * 3) : nullptr;
-  const uint4* aux4 = EPI != EPI_PLAIN ? reinterpret_cast<const uint4*>(a.aux) + (long)blk * a.aux_stride * (LS * 3) : nullptr;
-  const uint4* dot4 = (EPI == EPI_XPAY && a.dot_out) ? reinterpret_cast<const uint4*>(a.dotv) + (long)blk * a.dotv_stride * (LS * 3) : nullptr;
-  const uint32_t* lk32 = reinterpret_cast<const uint32_t*>(a.links) + (long)blk * a.link_stride * (4 * NG);
-  const uint8_t* flp = a.flip + (long)blk * a.link_stride;
+  // per-block-row base pointers (64-bit once per Dirichlet block); everything below is 32-bit offsets in units of uint4
+  const uint4 *in4, *aux4 = nullptr, *dot4 = nullptr;
+  uint4 *out4, *out24 = nullptr;
+  const uint32_t* lk32;
+  const uint8_t* flp;
   const int* nbr = a.nbr;
+  auto set_block = [&](int b) {
+    blk = b;
+    in4 = reinterpret_cast<const uint4*>(a.in) + (long)b * a.in_stride * (LS * 3);
+    out4 = reinterpret_cast<uint4*>(a.out) + (long)b * a.out_stride * (LS * 3);
+    if (EPI == EPI_K3) out24 = reinterpret_cast<uint4*>(a.out2) + (long)b * a.out2_stride * (LS * 3);
+    if (EPI != EPI_PLAIN) aux4 = reinterpret_cast<const uint4*>(a.aux) + (long)b * a.aux_stride * (LS * 3);
+    if (EPI == EPI_XPAY && a.dot_out) dot4 = reinterpret_cast<const uint4*>(a.dotv) + (long)b * a.dotv_stride * (LS * 3);
+    lk32 = reinterpret_cast<const uint32_t*>(a.links) + (long)b * a.link_stride * (4 * NG);
+    flp = a.flip + (long)b * a.link_stride;
+  };
 
   // lane constants: fragment offset inside a site column (pad lanes clamped onto valid data, they meet zeros in B)
   const int tt = t < 3 ? t : 2;
@@ -364,31 +371,39 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
     }
   };
 
+  // Thread blocks are persistent over Dirichlet blocks too (grid.y <= nblk): with thousands of small blocks (8^4 blocks of the
+  // 48^3 x 96 lattice) one wave of resident thread blocks walks all of them.  ph0 / ph1: parity of the next phase to wait for
+  // on the two stage barriers; an issue for a site past the end is an empty phase that nobody waits for and is skipped here.
   const int site0 = blockIdx.x * NW + warp;
-  Meta mA, mB;
-  ld_meta(site0, mA); ld_meta(site0 + stride, mB);
-  ld_aux(site0, mA); ld_aux(site0 + stride, mB);
-  issue(mA, 0);
-  uint32_t par = 0;
-  for (int site = site0; site < a.n_out; site += 2 * stride) {
-    step(site, 0, par, mA, mB);
-    if (site + stride < a.n_out) step(site + stride, 1, par, mB, mA);
-    par ^= 1u;
-  }
-  // drain: a copy set may still be in flight for a site past the end (only when its table was valid: never, the
-  // tables of sites >= n_out are -1, so the last issue carried zero bytes and completed at once)
+  uint32_t ph0 = 0, ph1 = 0;
+  for (int b = blockIdx.y; b < a.nblk; b += gridDim.y) {
+    set_block(b);
+    part = 0.f;
+    Meta mA, mB;
+    ld_meta(site0, mA); ld_meta(site0 + stride, mB);
+    ld_aux(site0, mA); ld_aux(site0 + stride, mB);
+    issue(mA, 0);
+    int nst = 0;
+    for (int site = site0; site < a.n_out; site += 2 * stride) {
+      step(site, 0, ph0, mA, mB); ph0 ^= 1u; nst++;
+      if (site + stride < a.n_out) { step(site + stride, 1, ph1, mB, mA); ph1 ^= 1u; nst++; }
+    }
+    if (nst == 0 || (nst & 1) == 0) ph0 ^= 1u; else ph1 ^= 1u;   // the trailing empty phase
+    __syncwarp();
 
-  if (EPI == EPI_XPAY) {
-    if (a.dot_out != nullptr) {
+    if (EPI == EPI_XPAY) {
+      if (a.dot_out != nullptr) {
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
-      if (lane == 0) red[warp] = (double)part;
-      __syncthreads();
-      if (threadIdx.x == 0) {
-        double tot = 0;
+        for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+        __syncthreads();                       // red[] of the previous Dirichlet block has been read
+        if (lane == 0) red[warp] = (double)part;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+          double tot = 0;
 #pragma unroll
-        for (int w = 0; w < NW; w++) tot += red[w];
-        atomicAdd(a.dot_out + (long)blk * a.dot_stride, tot);
+          for (int w = 0; w < NW; w++) tot += red[w];
+          atomicAdd(a.dot_out + (long)blk * a.dot_stride, tot);
+        }
       }
     }
   }

@@ -160,6 +160,7 @@ template <typename T> struct HopArgs {
   const int* nbr;                                  // [n_out][8], shared by all blocks
   const T* links; const uint8_t* flip; long link_stride;  // [blk][link_stride][8][ng], [blk][link_stride]
   int n_out, ng;
+  int nblk;                                        // fp16 path: Dirichlet blocks to walk (grid.y may be smaller)
   const C* mat1; const C* mat2;                    // device [2][LS][LS], transposed per chirality
   const uint4* frag1; const uint4* frag2;          // fp16 path: the same matrices as mma A fragments [2][32] (hop_mma.cuh)
   C sg;                                            // +1: D^w, -1: D^w^dag

@@ -223,11 +223,16 @@ cudaError_t launch_hop(mspcg_ctx* c, const HopArgs<T>& a, int nblk, cudaStream_t
       cudaFuncSetAttribute(k_hop_mma<LS, EPI, 12>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
       attr = true;
     }
-    int gx = (a.n_out + NW - 1) / NW, cap = (4 * c->num_sms) / nblk;   // persistent warps: one wave of <= 4 thread blocks per SM
+    // persistent warps: one wave of <= 4 thread blocks per SM, over the sites of a Dirichlet block (grid.x) and over blocks (grid.y)
+    const int slots = 4 * c->num_sms;
+    int gx = (a.n_out + NW - 1) / NW, cap = slots / nblk;
     if (gx > cap) gx = cap;
-    dim3 block(32 * NW), grid(gx < 1 ? 1 : gx, nblk);
+    if (gx < 1) gx = 1;
+    int gy = slots / gx; if (gy > nblk) gy = nblk; if (gy < 1) gy = 1;
+    dim3 block(32 * NW), grid(gx, gy);
+    HopArgs<__half> ab = a; ab.nblk = nblk;
     { TimedLaunch tl(c, kind, st);
-      if (a.ng == 12) k_hop_mma<LS, EPI, 12><<<grid, block, sm, st>>>(a); else k_hop_mma<LS, EPI, 18><<<grid, block, sm, st>>>(a); }
+      if (a.ng == 12) k_hop_mma<LS, EPI, 12><<<grid, block, sm, st>>>(ab); else k_hop_mma<LS, EPI, 18><<<grid, block, sm, st>>>(ab); }
   } else {
     static bool attr = false;
     const size_t sm = hop_smem<T, LS, EPI>();

@@ -289,3 +289,13 @@ def test_solve_fp16_sloppy_outer_iteration():
             x, s = g.solve(db, tol=1e-10, use_precond=pre, n_inner=5, sloppy_prec=F16, delta=0.1)
             assert s["rc"] == 0 and s["true_res"] <= 1e-10 and s["reliable_updates"] >= 5
             assert rel(x.cpu().numpy() / scale, x_ora) <= 1e-8
+
+
+def test_precond_fp16_more_blocks_than_resident_thread_blocks():
+    """864 Dirichlet blocks > 4 x 148 resident thread blocks: the fp16 hop kernel walks several blocks per thread block."""
+    dims, Ls, block = (12, 12, 12, 8), 4, (2, 2, 2, 2)
+    ora, g, torch = setup(dims, Ls, 0.02, block, outer=F32, inner=F16)
+    assert g.geometry()["nblk"] == 864
+    r = synth.gaussian_spinor_abi(dims, Ls, 19)
+    z = g.apply_precond(dev(torch, r), 3, F64).cpu().numpy()
+    assert rel(z, ora.apply_precond(r, 3)) <= 2e-2
