@@ -193,7 +193,7 @@ __device__ __forceinline__ void hop_dir(typename ST<T>::C* acc, const T* __restr
 }
 
 template <typename T, int LS, int EPI>
-__global__ void __launch_bounds__(Tile<LS>::NT, (sizeof(typename ST<T>::C) == 8 ? 2 : 3)) k_hop(const HopArgs<T> a) {
+__global__ void __launch_bounds__(Tile<LS>::NT, (sizeof(typename ST<T>::C) == 8 ? 4 : 5)) k_hop(const HopArgs<T> a) {
   typedef typename ST<T>::C C;
   typedef Smem<C, LS> SM;
   constexpr int NS = Tile<LS>::NS, NT = Tile<LS>::NT;
