@@ -48,6 +48,27 @@ class Oracle:
         f = mdwf.D_eo_dag if dagger else mdwf.D_eo
         return self.pack(f(self.mob, self.U, self.unpack(in_abi)))
 
+    # -- full 4-step solve (eq. 4-6, eq. 9) ----------------------------
+    def unpack_odd(self, v_abi):
+        return mdwf.unpack_spinor_abi(v_abi, self.dims, self.Ls, 1)
+
+    def pack_odd(self, v):
+        return mdwf.pack_spinor_abi(v, self.dims, 1)
+
+    def prepare_source(self, phi_e_abi, phi_o_abi):
+        """(phihat_e of eq. 6, D^dag phihat_e of eq. 9), both even-parity ABI vectors."""
+        pe, po = self.unpack(phi_e_abi), self.unpack_odd(phi_o_abi)
+        hat = mdwf.prepare_source(self.mob, self.U, pe, po)
+        return self.pack(hat), self.pack(mdwf.D_eo_dag(self.mob, self.U, hat))
+
+    def reconstruct_odd(self, psi_e_abi, phi_o_abi):
+        return self.pack_odd(mdwf.reconstruct_odd(self.mob, self.U, self.unpack(psi_e_abi), self.unpack_odd(phi_o_abi)))
+
+    def apply_full(self, psi_e_abi, psi_o_abi):
+        """The unpreconditioned 2x2 operator of eq. (4) -> (even part, odd part)."""
+        out = mdwf.D_dw(self.mob, self.U, self.unpack(psi_e_abi) + self.unpack_odd(psi_o_abi))
+        return self.pack(out), self.pack_odd(out)
+
     def apply_precond(self, r_abi, n_inner, variant="PAD", blocks=None):
         return self.pack(self.precond_obj(variant)(self.unpack(r_abi), n_inner, blocks))
 

@@ -266,6 +266,35 @@ def MdagM(mob, U, psi_e, periodic=(True,) * 4):
 
 
 # ---------------------------------------------------------------------------
+# Full 4-step solve.  PAPER.md:89-97: the 2x2 system of eq. (4),
+#   [[M5, M4eo], [M4oe, M5]] (psi_e, psi_o) = (phi_e, phi_o),
+# is solved through eq. (5) D psi_e = phihat_e with the prepared source of eq. (6),
+#   phihat_e = M5^-1 phi_e - M5^-1 M4eo M5^-1 phi_o,
+# the normal equations of eq. (9), D^dag D psi_e = D^dag phihat_e, and the second row of
+# eq. (4) for the odd sites, psi_o = M5^-1 (phi_o - M4oe psi_e).  M4 = D^w Mphi (eq. 7).
+# Fields carry both parities (the unused one zero), so phi = phi_e + phi_o needs no index code.
+# ---------------------------------------------------------------------------
+def M4(mob, U, psi):
+    """M4eo / M4oe of eq. (7): the hop flips the parity of whatever it is given."""
+    return hop(U, Mphi(mob, psi))
+
+
+def prepare_source(mob, U, phi_e, phi_o):
+    """eq. (6): phihat_e."""
+    return M5inv(mob, phi_e) - M5inv(mob, M4(mob, U, M5inv(mob, phi_o)))
+
+
+def normal_rhs(mob, U, phi_e, phi_o):
+    """eq. (9): right-hand side D^dag phihat_e of the CGNR system."""
+    return D_eo_dag(mob, U, prepare_source(mob, U, phi_e, phi_o))
+
+
+def reconstruct_odd(mob, U, psi_e, phi_o):
+    """Second row of eq. (4): psi_o = M5^-1 (phi_o - M4oe psi_e)."""
+    return M5inv(mob, phi_o - M4(mob, U, psi_e))
+
+
+# ---------------------------------------------------------------------------
 # Dirichlet block operator A_s with snake terms.
 # PAD (binding reading R10; PAPER.md:224): "the vector is padded in both directions of each
 # partitioned dimension by size of two ... the pad region is initialized to zero.  The operators
