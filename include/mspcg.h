@@ -96,6 +96,19 @@ int mspcg_apply_precond_host(mspcg_ctx* ctx, const double* r_host, double* z_hos
  * out is zero outside the block. */
 int mspcg_apply_A_block(mspcg_ctx* ctx, const double* in_dev, double* out_dev, int block, int prec, void* stream);
 
+/* Full 4-step solve: the set-up and tear-down around mspcg_solve for the unpreconditioned system of
+ * PAPER.md:91 eq. (4), [[M5, M4eo],[M4oe, M5]] (psi_e, psi_o) = (phi_e, phi_o).  All vectors DEVICE fp64, ABI layout; an
+ * ODD-parity vector is psi[s][x_cb][4][3][re,im] with x_cb = lex(x,y,z,t; x fastest)/2 over the odd sites.  fp64 arithmetic.
+ *   mspcg_prepare_source:  phihat_e = M5^-1 phi_e - M5^-1 M4eo M5^-1 phi_o (eq. 6) -> phihat_e_dev (or NULL),
+ *                          rhs = D^dag phihat_e (eq. 9) -> rhs_dev, the `b` of mspcg_solve;
+ *   mspcg_reconstruct_odd: psi_o = M5^-1 (phi_o - M4oe psi_e) (second row of eq. 4) from the solution psi_e of mspcg_solve;
+ *   mspcg_apply_full:      (out_e, out_o) = the 2x2 operator of eq. (4) applied to (psi_e, psi_o), to check a solution.
+ * They use the solver's vectors as scratch (do not run concurrently with mspcg_solve on another stream).  Outputs may not
+ * alias inputs.  Errors: MSPCG_EINVAL (null pointer), MSPCG_ENOGAUGE / MSPCG_ENOWORKSPACE, MSPCG_ECUDA. */
+int mspcg_prepare_source(mspcg_ctx* ctx, const double* phi_e_dev, const double* phi_o_dev, double* phihat_e_dev, double* rhs_dev, void* stream);
+int mspcg_reconstruct_odd(mspcg_ctx* ctx, const double* psi_e_dev, const double* phi_o_dev, double* psi_o_dev, void* stream);
+int mspcg_apply_full(mspcg_ctx* ctx, const double* psi_e_dev, const double* psi_o_dev, double* out_e_dev, double* out_o_dev, void* stream);
+
 /* Reduced-Ls preconditioner: Ls_hat in {4,6,8,12,16}, Ls_hat <= Ls; T_host[4*Ls_hat][4*Ls][re,im]
  * (HOST, copied; row (s_hat,spin), column (s,spin); identity in colour and 4D site, eq. 21), shift mu (eq. 20).  The
  * reduced operator uses the same b, c, M5, mf (reading R19).  Must be called before mspcg_workspace_bytes.  Afterwards

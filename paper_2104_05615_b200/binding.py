@@ -24,6 +24,7 @@ SYMBOLS = [
     "mspcg_unpack", "mspcg_apply_MdagM", "mspcg_apply_precond", "mspcg_apply_MdagM_host",
     "mspcg_apply_precond_host", "mspcg_apply_A_block", "mspcg_set_reduced_ls", "mspcg_solve", "mspcg_launch_count",
     "mspcg_timing", "mspcg_timing_read", "mspcg_update_T", "mspcg_train_eval", "mspcg_train_T",
+    "mspcg_prepare_source", "mspcg_reconstruct_odd", "mspcg_apply_full",
 ]
 
 
@@ -69,6 +70,9 @@ def load_library():
     L.mspcg_apply_MdagM_host.argtypes = [vp, vp, vp, i]
     L.mspcg_apply_precond_host.argtypes = [vp, vp, vp, i, i, i]
     L.mspcg_apply_A_block.argtypes = [vp, vp, vp, i, i, vp]
+    L.mspcg_prepare_source.argtypes = [vp, vp, vp, vp, vp, vp]
+    L.mspcg_reconstruct_odd.argtypes = [vp, vp, vp, vp, vp]
+    L.mspcg_apply_full.argtypes = [vp, vp, vp, vp, vp, vp]
     L.mspcg_set_reduced_ls.argtypes = [vp, i, dp, d]
     L.mspcg_solve.argtypes = [vp, vp, vp, C.POINTER(SolveParams), C.POINTER(SolveStats), vp]
     L.mspcg_launch_count.argtypes = [vp]
@@ -241,6 +245,28 @@ class Mspcg:
         self._check(self.lib.mspcg_apply_A_block(self.h, C.c_void_p(v_abi.data_ptr()), C.c_void_p(out.data_ptr()), int(block),
                                                  prec if prec is not None else self.inner_prec, self._stream()))
         return out
+
+    def prepare_source(self, phi_e_abi, phi_o_abi):
+        """(phihat_e, D^dag phihat_e) of PAPER.md:97 eq. 6 and PAPER.md:117 eq. 9; fp64 ABI device tensors."""
+        torch = _torch()
+        hat, rhs = torch.empty_like(phi_e_abi), torch.empty_like(phi_e_abi)
+        self._check(self.lib.mspcg_prepare_source(self.h, C.c_void_p(phi_e_abi.data_ptr()), C.c_void_p(phi_o_abi.data_ptr()),
+                                                  C.c_void_p(hat.data_ptr()), C.c_void_p(rhs.data_ptr()), self._stream()))
+        return hat, rhs
+
+    def reconstruct_odd(self, psi_e_abi, phi_o_abi):
+        torch = _torch()
+        out = torch.empty_like(phi_o_abi)
+        self._check(self.lib.mspcg_reconstruct_odd(self.h, C.c_void_p(psi_e_abi.data_ptr()), C.c_void_p(phi_o_abi.data_ptr()),
+                                                   C.c_void_p(out.data_ptr()), self._stream()))
+        return out
+
+    def apply_full(self, psi_e_abi, psi_o_abi):
+        torch = _torch()
+        oe, oo = torch.empty_like(psi_e_abi), torch.empty_like(psi_o_abi)
+        self._check(self.lib.mspcg_apply_full(self.h, C.c_void_p(psi_e_abi.data_ptr()), C.c_void_p(psi_o_abi.data_ptr()),
+                                              C.c_void_p(oe.data_ptr()), C.c_void_p(oo.data_ptr()), self._stream()))
+        return oe, oo
 
     def apply_MdagM_host(self, v_host, out_host, prec=F64):
         self._check(self.lib.mspcg_apply_MdagM_host(self.h, C.c_void_p(v_host.data_ptr()), C.c_void_p(out_host.data_ptr()), prec))

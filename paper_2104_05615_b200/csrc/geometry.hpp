@@ -40,6 +40,7 @@ struct Lattice {
   long V4;
   Geometry blk, full;
   std::vector<int> e_int_to_cb;    // FULL E-list index -> ABI x_cb (even parity)
+  std::vector<int> o_int_to_cb;    // FULL O-list index -> ABI x_cb (odd parity)
 };
 
 inline int pmod(int a, int m) { int r = a % m; return r < 0 ? r + m : r; }
@@ -105,7 +106,7 @@ inline void build_full_geometry(Lattice& lat) {
   g.origin.assign(4, 0);
   g.cE.resize((size_t)Vh * 4); g.cO.resize((size_t)Vh * 4);
   std::vector<int> lex2int(lat.V4, -1);
-  lat.e_int_to_cb.resize(Vh);
+  lat.e_int_to_cb.resize(Vh); lat.o_int_to_cb.resize(Vh);
   auto lexof = [&](const int c[4]) { return c[0] + (long)lat.L[0] * (c[1] + (long)lat.L[1] * (c[2] + (long)lat.L[2] * c[3])); };
   for (int b = 0; b < lat.nblk; b++) {
     const short* o = &bg.origin[4 * b];
@@ -119,7 +120,7 @@ inline void build_full_geometry(Lattice& lat) {
       int c[4]; for (int d = 0; d < 4; d++) c[d] = o[d] + bg.cO[4 * i + d];
       long k = (long)b * bg.nO0 + i;
       for (int d = 0; d < 4; d++) g.cO[4 * k + d] = (short)c[d];
-      lex2int[lexof(c)] = (int)k;
+      lex2int[lexof(c)] = (int)k; lat.o_int_to_cb[k] = (int)(lexof(c) / 2);
     }
   }
   auto neighbours = [&](const std::vector<short>& cs, long n, std::vector<int>& out) {

@@ -148,6 +148,31 @@ __device__ __forceinline__ void dense5d(const C* __restrict__ slab_j, const C* _
   }
 }
 
+// Stand-alone fifth-dimension matrix, out = M in on n_sites site columns (set-up steps of the full solve: the M5^-1
+// factors of the prepared source, eq. 6, that are not preceded by a hop).  mat: [2][LS][LS] transposed per
+// chirality like HopArgs::mat1.
+template <typename T, int LS>
+__global__ void __launch_bounds__(Tile<LS>::NT) k_dense5d(const T* __restrict__ in, T* __restrict__ out, const typename ST<T>::C* __restrict__ mat, long n_sites) {
+  typedef typename ST<T>::C C;
+  typedef Smem<C, LS> SM;
+  constexpr int NS = Tile<LS>::NS;
+  extern __shared__ __align__(16) unsigned char smraw[];
+  C* slab = reinterpret_cast<C*>(smraw);
+  C* Msm = slab + NS * SM::SSTRIDE;
+  const int s = threadIdx.x, j = threadIdx.y;
+  for (int i = j * LS + s; i < 2 * LS * LS; i += NS * LS) Msm[i] = mat[i];
+  const long site = (long)blockIdx.x * NS + j;
+  const bool live = site < n_sites;
+  C v[24], o[24];
+  load24_pred<T>(in, live ? site : 0, s, LS, live, v);
+  C* slab_j = slab + j * SM::SSTRIDE;
+#pragma unroll
+  for (int k = 0; k < 24; k++) slab_j[k * LS + s] = v[k];
+  __syncthreads();
+  dense5d<C, LS>(slab_j, Msm, s, o);
+  if (live) store24<T>(out, site, s, LS, o);
+}
+
 // ------------------------------------------------------------------------------------------ fused hop kernel (A3+A4)
 template <typename T> struct HopArgs {
   typedef typename ST<T>::C C;

@@ -73,7 +73,8 @@ struct mspcg_ctx {
   size_t ws_bytes = 0;
   // device
   GeomDev gfull, gblk;
-  int* e_int_to_cb = nullptr;
+  int *e_int_to_cb = nullptr, *o_int_to_cb = nullptr;   // FULL list index -> ABI x_cb, even / odd parity
+  double* negI = nullptr;        // device [2][Ls][Ls]: minus the identity (full 2x2 operator of eq. 4, mspcg_apply_full)
   MatSet<double> md, md_hat; MatSet<float> mf32, mf32_hat; MatFrag mfr, mfr_hat;
   OpBuf full64, fullS, blkI;     // full lattice fp64 / sloppy; block geometry in the inner precision
   void *in_r = nullptr, *in_p = nullptr, *in_q = nullptr, *in_x = nullptr;   // inner CG vectors [V5h]
@@ -157,7 +158,8 @@ void carve_temps(Arena& a, OpBuf& o, const Geometry& g, int Ls) {   // stage vec
 void carve(mspcg_ctx* c, Arena& a) {
   const Lattice& L = c->lat;
   carve_geom(a, c->gfull, L.full); carve_geom(a, c->gblk, L.blk);
-  c->e_int_to_cb = a.take<int>(L.e_int_to_cb.size());
+  c->e_int_to_cb = a.take<int>(L.e_int_to_cb.size()); c->o_int_to_cb = a.take<int>(L.o_int_to_cb.size());
+  c->negI = a.take<double>((size_t)2 * c->Ls * c->Ls);
   carve_mats(a, c->md, c->Ls); carve_mats(a, c->mf32, c->Ls); carve_frags(a, c->mfr);
   if (c->Ls_hat) { carve_mats(a, c->md_hat, c->Ls_hat); carve_mats(a, c->mf32_hat, c->Ls_hat); carve_frags(a, c->mfr_hat); }
   c->rho = a.take<double>((size_t)(KMAX + 1) * L.nblk); c->pq = a.take<double>((size_t)KMAX * L.nblk);
@@ -453,10 +455,11 @@ cudaError_t normal_full_any(mspcg_ctx* c, int prec, const void* p, void* q, doub
   return normal_full<__half>(c, *ob, (const __half*)p, (__half*)q, mphi_plain<__half>((const __half*)p), dot_out, st);
 }
 
-cudaError_t pack_any(mspcg_ctx* c, const double* abi, void* nat, int prec, int to_native, cudaStream_t st) {
+cudaError_t pack_any(mspcg_ctx* c, const double* abi, void* nat, int prec, int to_native, cudaStream_t st, int parity = 0) {
   const long Vh = c->lat.V4 / 2;
+  const int* table = parity ? c->o_int_to_cb : c->e_int_to_cb;
 #define PK(TT) DISPATCH_LS(c->Ls, { dim3 block(LS, Tile<LS>::NS), grid((unsigned)((Vh + Tile<LS>::NS - 1) / Tile<LS>::NS)); \
-    k_pack<TT, LS><<<grid, block, 0, st>>>(abi, (TT*)nat, c->e_int_to_cb, Vh, to_native); })
+    k_pack<TT, LS><<<grid, block, 0, st>>>(abi, (TT*)nat, table, Vh, to_native); })
   if (prec == MSPCG_F64) PK(double) else if (prec == MSPCG_F32) PK(float) else PK(__half)
 #undef PK
   c->launches++;
@@ -565,6 +568,75 @@ template <typename T> cudaError_t axpby(mspcg_ctx* c, double a, const T* x, doub
   k_axpby<T><<<(unsigned)((nchunk + 255) / 256), 256, 0, st>>>(a, x, b, y, nchunk);
   c->launches++;
   return cudaPeekAtLastError();
+}
+
+// ------------------------------------------------------------------ full 4-step solve: set-up and tear-down
+// fp64 on the FULL geometry.  PAPER.md:89-97: eq. (4) [[M5, M4eo],[M4oe, M5]](psi_e, psi_o) = (phi_e, phi_o), M4 = D^w Mphi (eq. 7).
+template <int LS>
+cudaError_t dense_full64(mspcg_ctx* c, const double* in, double* out, const double* mat, cudaStream_t st) {
+  typedef Smem<double, LS> SM;
+  static bool attr = false;
+  const size_t sm = sizeof(double) * ((size_t)SM::NS * SM::SSTRIDE + (size_t)2 * LS * LS);
+  if (!attr) { cudaFuncSetAttribute(k_dense5d<double, LS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); attr = true; }
+  const long n = c->lat.V4 / 2;
+  dim3 block(LS, Tile<LS>::NS), grid((unsigned)((n + Tile<LS>::NS - 1) / Tile<LS>::NS));
+  k_dense5d<double, LS><<<grid, block, sm, st>>>(in, out, mat, n);
+  c->launches++;
+  return cudaPeekAtLastError();
+}
+// out = mat * D^w(^dag) in (EPI_PLAIN)  or  out = aux - mat * D^w(^dag) in (EPI_XPAY); to_odd: `in` on even sites, `out` on odd ones.
+template <int LS, int EPI>
+cudaError_t hop_full64(mspcg_ctx* c, const double* in, double* out, const double* aux, const double* mat, bool to_odd, double sg, cudaStream_t st) {
+  const Geometry& g = c->lat.full; const OpBuf& o = c->full64;
+  HopArgs<double> a; memset(&a, 0, sizeof(a));
+  a.ng = o.ng; a.in = in; a.in_stride = g.nE; a.n_in_limit = g.nE; a.out = out; a.out_stride = g.nE; a.n_out = g.nE;
+  a.aux = aux; a.aux_stride = g.nE; a.n_aux = aux ? g.nE : 0;
+  a.nbr = to_odd ? c->gfull.nbrO : c->gfull.nbrE; a.links = (const double*)(to_odd ? o.linksO : o.linksE); a.flip = to_odd ? o.flipO : o.flipE;
+  a.link_stride = g.nE; a.mat1 = mat; a.sg = sg;
+  return launch_hop<double, LS, EPI>(c, a, 1, st);
+}
+template <int LS>
+cudaError_t bidiag_full64(mspcg_ctx* c, const double* in, double* out, double diag, double off, cudaStream_t st) {
+  MphiArgs<double> mp = mphi_plain<double>(in);
+  mp.t = out; mp.n_sites = c->lat.V4 / 2; mp.diag = diag; mp.off = off; mp.mf = c->mf;
+  return launch_mphi<double, LS>(c, mp, 1, st);
+}
+// phihat_e = M5^-1 phi_e - M5^-1 M4eo M5^-1 phi_o (eq. 6) -> hat;  rhs = D^dag phihat_e (eq. 9).  pe, po, hat, rhs: NATIVE fp64.
+template <int LS>
+cudaError_t prepare_source_impl(mspcg_ctx* c, const double* pe, const double* po, double* hat, double* rhs, cudaStream_t st) {
+  const MatSet<double>& m = c->md; const OpBuf& o = c->full64;
+  double *t1 = (double*)o.t1, *tO = (double*)o.tO, *w = (double*)o.w;
+  cudaError_t e;
+  if ((e = dense_full64<LS>(c, po, tO, m.K2, st)) != cudaSuccess) return e;                                  // Mphi M5^-1 phi_o
+  if ((e = dense_full64<LS>(c, pe, t1, m.K3a, st)) != cudaSuccess) return e;                                 // M5^-1 phi_e
+  if ((e = hop_full64<LS, EPI_XPAY>(c, tO, hat, t1, m.K3a, false, 1.0, st)) != cudaSuccess) return e;        // - M5^-1 D^w (.)
+  if ((e = dense_full64<LS>(c, hat, w, m.K3b, st)) != cudaSuccess) return e;                                 // D^dag: M5^-dag
+  if ((e = hop_full64<LS, EPI_PLAIN>(c, w, tO, nullptr, m.K4, true, -1.0, st)) != cudaSuccess) return e;     //   (M5^-dag Mphi^dag) D^w^dag
+  return hop_full64<LS, EPI_XPAY>(c, tO, rhs, hat, m.K5, false, -1.0, st);                                   //   1 - Mphi^dag D^w^dag (.)
+}
+// psi_o = M5^-1 (phi_o - M4oe psi_e) (second row of eq. 4).  NATIVE fp64.
+template <int LS>
+cudaError_t reconstruct_odd_impl(mspcg_ctx* c, const double* xe, const double* po, double* xo, cudaStream_t st) {
+  const MatSet<double>& m = c->md; const OpBuf& o = c->full64;
+  double *t1 = (double*)o.t1, *w = (double*)o.w;
+  cudaError_t e;
+  if ((e = bidiag_full64<LS>(c, xe, t1, c->hm.diag, c->hm.off, st)) != cudaSuccess) return e;                // Mphi psi_e
+  if ((e = dense_full64<LS>(c, po, w, m.K3a, st)) != cudaSuccess) return e;                                  // M5^-1 phi_o
+  return hop_full64<LS, EPI_XPAY>(c, t1, xo, w, m.K3a, true, 1.0, st);                                       // - M5^-1 D^w (.)
+}
+// (out_e, out_o) = the 2x2 operator of eq. 4 on (psi_e, psi_o).  NATIVE fp64.
+template <int LS>
+cudaError_t apply_full_impl(mspcg_ctx* c, const double* xe, const double* xo, double* oe, double* oo, cudaStream_t st) {
+  const OpBuf& o = c->full64;
+  double *t1 = (double*)o.t1, *y = (double*)o.y;
+  cudaError_t e;
+  for (int par = 0; par < 2; par++) {   // out_par = M5 psi_par + D^w Mphi psi_other
+    const double *same = par ? xo : xe, *other = par ? xe : xo;
+    if ((e = bidiag_full64<LS>(c, same, y, c->alpha, c->beta, st)) != cudaSuccess) return e;
+    if ((e = bidiag_full64<LS>(c, other, t1, c->hm.diag, c->hm.off, st)) != cudaSuccess) return e;
+    if ((e = hop_full64<LS, EPI_XPAY>(c, t1, par ? oo : oe, y, c->negI, par != 0, 1.0, st)) != cudaSuccess) return e;
+  }
+  return cudaSuccess;
 }
 
 // ------------------------------------------------------------------------------------------------ outer PCG (A11)
@@ -860,7 +932,10 @@ int mspcg_set_workspace(mspcg_ctx* ctx, void* workspace_dev, size_t bytes, void*
   CUDA_OK(ctx, up(ctx->gblk.nbrE, L.blk.nbrE, st)); CUDA_OK(ctx, up(ctx->gblk.nbrO, L.blk.nbrO, st));
   CUDA_OK(ctx, up(ctx->gblk.cE, L.blk.cE, st)); CUDA_OK(ctx, up(ctx->gblk.cO, L.blk.cO, st));
   CUDA_OK(ctx, up(ctx->gblk.origin, L.blk.origin, st));
-  CUDA_OK(ctx, up(ctx->e_int_to_cb, L.e_int_to_cb, st));
+  CUDA_OK(ctx, up(ctx->e_int_to_cb, L.e_int_to_cb, st)); CUDA_OK(ctx, up(ctx->o_int_to_cb, L.o_int_to_cb, st));
+  { std::vector<double> ni((size_t)2 * ctx->Ls * ctx->Ls, 0.0);
+    for (int ch = 0; ch < 2; ch++) for (int i = 0; i < ctx->Ls; i++) ni[((size_t)ch * ctx->Ls + i) * ctx->Ls + i] = -1.0;
+    CUDA_OK(ctx, up(ctx->negI, ni, st)); }
   CUDA_OK(ctx, cudaStreamSynchronize(st));
   CUDA_OK(ctx, upload_mats<double>(ctx->md, ctx->hm, st)); CUDA_OK(ctx, upload_mats<float>(ctx->mf32, ctx->hm, st));
   CUDA_OK(ctx, upload_frags(ctx->mfr, ctx->hm, ctx->Ls, st));
@@ -929,6 +1004,42 @@ int mspcg_apply_precond(mspcg_ctx* ctx, const void* r_dev, void* z_dev, int io_p
     CUDA_OK(ctx, precond_any(ctx, ctx->stage_in, ctx->stage_out, io_prec, n_inner, use_reduced != 0, st));
     CUDA_OK(ctx, pack_any(ctx, (double*)z_dev, ctx->stage_out, io_prec, 0, st));
   }
+  return MSPCG_OK;
+}
+
+int mspcg_prepare_source(mspcg_ctx* ctx, const double* phi_e_dev, const double* phi_o_dev, double* phihat_e_dev, double* rhs_dev, void* stream) {
+  int rc = check_ready(ctx, true); if (rc) return rc;
+  if (!phi_e_dev || !phi_o_dev || !rhs_dev) return fail(ctx, MSPCG_EINVAL, "null pointer");
+  cudaStream_t st = (cudaStream_t)stream;
+  double *pe = ctx->v_b, *po = ctx->v_xhi, *hat = ctx->v_rhi, *rhs = ctx->v_t64;
+  CUDA_OK(ctx, pack_any(ctx, phi_e_dev, pe, MSPCG_F64, 1, st, 0));
+  CUDA_OK(ctx, pack_any(ctx, phi_o_dev, po, MSPCG_F64, 1, st, 1));
+  DISPATCH_LS(ctx->Ls, CUDA_OK(ctx, (prepare_source_impl<LS>(ctx, pe, po, hat, rhs, st))));
+  if (phihat_e_dev) CUDA_OK(ctx, pack_any(ctx, phihat_e_dev, hat, MSPCG_F64, 0, st, 0));
+  CUDA_OK(ctx, pack_any(ctx, rhs_dev, rhs, MSPCG_F64, 0, st, 0));
+  return MSPCG_OK;
+}
+int mspcg_reconstruct_odd(mspcg_ctx* ctx, const double* psi_e_dev, const double* phi_o_dev, double* psi_o_dev, void* stream) {
+  int rc = check_ready(ctx, true); if (rc) return rc;
+  if (!psi_e_dev || !phi_o_dev || !psi_o_dev) return fail(ctx, MSPCG_EINVAL, "null pointer");
+  cudaStream_t st = (cudaStream_t)stream;
+  double *xe = ctx->v_b, *po = ctx->v_xhi, *xo = ctx->v_rhi;
+  CUDA_OK(ctx, pack_any(ctx, psi_e_dev, xe, MSPCG_F64, 1, st, 0));
+  CUDA_OK(ctx, pack_any(ctx, phi_o_dev, po, MSPCG_F64, 1, st, 1));
+  DISPATCH_LS(ctx->Ls, CUDA_OK(ctx, (reconstruct_odd_impl<LS>(ctx, xe, po, xo, st))));
+  CUDA_OK(ctx, pack_any(ctx, psi_o_dev, xo, MSPCG_F64, 0, st, 1));
+  return MSPCG_OK;
+}
+int mspcg_apply_full(mspcg_ctx* ctx, const double* psi_e_dev, const double* psi_o_dev, double* out_e_dev, double* out_o_dev, void* stream) {
+  int rc = check_ready(ctx, true); if (rc) return rc;
+  if (!psi_e_dev || !psi_o_dev || !out_e_dev || !out_o_dev) return fail(ctx, MSPCG_EINVAL, "null pointer");
+  cudaStream_t st = (cudaStream_t)stream;
+  double *xe = ctx->v_b, *xo = ctx->v_xhi, *oe = ctx->v_rhi, *oo = ctx->v_t64;
+  CUDA_OK(ctx, pack_any(ctx, psi_e_dev, xe, MSPCG_F64, 1, st, 0));
+  CUDA_OK(ctx, pack_any(ctx, psi_o_dev, xo, MSPCG_F64, 1, st, 1));
+  DISPATCH_LS(ctx->Ls, CUDA_OK(ctx, (apply_full_impl<LS>(ctx, xe, xo, oe, oo, st))));
+  CUDA_OK(ctx, pack_any(ctx, out_e_dev, oe, MSPCG_F64, 0, st, 0));
+  CUDA_OK(ctx, pack_any(ctx, out_o_dev, oo, MSPCG_F64, 0, st, 1));
   return MSPCG_OK;
 }
 
