@@ -366,10 +366,20 @@ def extras(torch, g, cfg, U, src, d_src, geo, peak, args):
     torch.cuda.empty_cache()
     # reduced-Ls preconditioner: T trained with the library (eq. 22; set-up step, its time reported, not
     # part of the solve) on residual vectors of a full-Ls MSPCG run, then MSPCG with z = T^dag CG_k[Mhat](T r) + mu r
+    # T is the identity in 4D site and colour (eq. 21), so it is trained on a sample lattice of at most 16^3 x 32 sites with the same
+    # Moebius parameters, mass and link roughness (its own seeds) and Dirichlet blocks of at most half its extent, and then
+    # used on the full lattice -- the paper likewise trains once per ensemble.
     from paper_2104_05615_b200.train_reduced_ls import train
-    Lh, mu = cfg.get("Ls_hat", Ls // 2), 0.3
+    Lh, mu = cfg.get("Ls_hat", Ls // 2), args.mu
+    tdims = tuple(min(d, 16 if i < 3 else 32) for i, d in enumerate(dims))
+    tblock = tuple(min(b, t // 2) if b < d else t for b, t, d in zip(block, tdims, dims))
+    if tdims == tuple(dims):
+        U_t, src_t, tblock = U, src, block
+    else:
+        U_t = synth.gauge_natural_to_abi(synth.random_su3_links(tdims, cfg["eps"], cfg["gauge_seed"] + 100), tdims)
+        src_t = synth.gaussian_spinor_abi(tdims, Ls, cfg["src_seed"] + 100)
     t0 = time.time()
-    T, info = train(dims, Ls, dict(b=cfg["b"], c=cfg["c"], M5=cfg["M5"]), cfg["mf"], block, U, src, Lh, mu, k,
+    T, info = train(tdims, Ls, dict(b=cfg["b"], c=cfg["c"], M5=cfg["M5"]), cfg["mf"], tblock, U_t, src_t, Lh, mu, k,
                     n_vec=12, span=120, n_steps=args.train_steps, momentum=0.5)
     torch.cuda.synchronize()
     train_s = time.time() - t0
@@ -380,8 +390,8 @@ def extras(torch, g, cfg, U, src, d_src, geo, peak, args):
     v, o = gr.pack(d_src, F32), gr.new_native(F32)
     ms = timed(torch, lambda: gr.apply_precond(v, k, F32, LAYOUT_NATIVE, out=o, use_reduced=1), steps, warm) / steps
     x, s = gr.solve(d_src, tol=1e-10, max_iter=200000, use_precond=True, n_inner=k, sloppy_prec=F32, delta=0.1, use_reduced_ls=True)
-    ex["reducedLs%d_trainedT_mu%.1f" % (Lh, mu)] = dict(
-        Mpre_ms=ms, train_seconds=train_s, train_steps=args.train_steps, chi2_first=float(info["chi2"][0]), chi2_last=float(info["chi2"][-1]),
+    ex["reducedLs%d_trainedT_mu%.2f" % (Lh, mu)] = dict(
+        Mpre_ms=ms, train_seconds=train_s, train_steps=args.train_steps, train_lattice=list(tdims), train_block=list(tblock), chi2_first=float(info["chi2"][0]), chi2_last=float(info["chi2"][-1]),
         solve=dict(seconds=s["seconds"], outer_iters=s["iters"], reliable_updates=s["reliable_updates"],
                    inner_applies=s["inner_applies"], true_res=s["true_res"], rc=s["rc"]))
     del x, v, o
@@ -399,8 +409,9 @@ def extras(torch, g, cfg, U, src, d_src, geo, peak, args):
     g3.configure(F16, F16, 18)
     g3.load_gauge(U, -1)
     sol = {}
+    cap = 3 * ex["solve_tol1e-10_fp32outer_fp16inner"]["CG"]["outer_iters"]   # plain fp16 CG can stagnate on ill-conditioned systems (rc = ENOCONV then)
     for name, pre in (("CG", False), ("MSPCG", True)):
-        x, s = g3.solve(d_src, tol=1e-10, max_iter=200000, use_precond=pre, n_inner=k, sloppy_prec=F16, delta=0.1)
+        x, s = g3.solve(d_src, tol=1e-10, max_iter=cap, use_precond=pre, n_inner=k, sloppy_prec=F16, delta=0.1)
         sol[name] = dict(seconds=s["seconds"], outer_iters=s["iters"], reliable_updates=s["reliable_updates"],
                          inner_applies=s["inner_applies"], true_res=s["true_res"], rc=s["rc"])
     ex["solve_tol1e-10_fp16outer_fp16inner"] = sol
@@ -480,7 +491,8 @@ def main():
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--block", default="", help="override the Dirichlet block, e.g. 12,12,12,12 (C5 block-size sweep)")
     ap.add_argument("--recon", type=int, default=18, choices=[12, 18], help="link storage of the low-precision copies (12 = two rows, R8)")
-    ap.add_argument("--train-steps", type=int, default=40, help="line-search steps of the T training in the extras")
+    ap.add_argument("--train-steps", type=int, default=100, help="line-search steps of the T training in the extras")
+    ap.add_argument("--mu", type=float, default=0.85, help="shift mu of the reduced-Ls preconditioner in the extras (PAPER.md:309 eq. 20; the paper's tuned values: 0.437-0.85)")
     ap.add_argument("--reduced", type=int, default=0, help="profiling aid: run the step with the reduced-Ls preconditioner at this Ls_hat")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
