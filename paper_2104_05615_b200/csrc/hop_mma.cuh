@@ -1,19 +1,20 @@
 // hop_mma.cuh -- the fused hop kernel for fp16 storage (the preconditioner's hot path): one WARP
-// owns one 4D site and its whole fifth-dimension column; the SU(3) x spinor products and the Ls x Ls fifth-dimension
-// contractions both run on the tensor cores with fp16 operands (exactly the stored values) and fp32 accumulation,
-// so the only CUDA-core arithmetic left is the gamma-matrix recombination (64 FMAs per site column) and conversions.
+// owns one 4D site and its whole fifth-dimension column; the SU(3) x half-spinor products and the Ls x Ls fifth-dimension
+// contractions both run on the tensor cores with fp16 operands and fp32 accumulation; the CUDA cores do the spin
+// projection (packed fp16 adds), the reconstruction of the lower components (32 FMAs per site column) and conversions.
 //
 // fp16 vector layout in HBM (private NATIVE layout of the __half storage type, see ST<__half> in kernels.cuh):
 //     v[site][s][colour t (3)][sp (2)][hi (2)][re,im]          spin = 2*hi + sp   (hi = 0: P+ rows, hi = 1: P- rows)
 // i.e. 48 contiguous bytes per (site, s), three 16-byte chunks, one per colour.  Lane (g = lane/4, t = lane%4) of the
-// warp loads the chunk of colour t for s = g and s = 8 + g: two 128-bit loads that ARE the A fragments of
-// mma.m16n8k16 for the four M-tiles (seg = s/8, sp) with rows (hi, g) and K = (colour, re/im) (lanes t = 3 pad K with
-// zeros).  The B fragment is the link as a real 6x6 (padded 8x8) matrix, built from one 32-bit load per lane.
+// warp reads the chunk {u0, l0, u1, l1} of colour t for s = g and s = 8 + g (u = upper, l = lower two-spinor).
 //
-//   hop (eq. 8):   sum_d (1 + sigma_d gamma_mu) W_d psi_d  =  S + sg * sum_mu gamma_mu Delta_mu,
-//       S = sum_d W_d psi_d (accumulated in one fragment set over all eight directions),
-//       Delta_mu = W_b psi_b - W_f psi_f (one k=16 MMA per M-tile: forward and backward neighbour side by side in K,
-//       the forward half of B negated), and gamma_mu only permutes (sp, hi) and swaps re/im inside a lane.
+//   hop (eq. 8), per direction:  (1 + c gamma_mu) W psi,  c = -sg (forward), +sg (backward), W the link.
+//       In the chiral basis (reading R2) its upper part is W h with the half spinor h = u + c G l (G = -i sigma_k, 1 for
+//       mu = t) and its lower part is c G^dag (W h).  h is formed in the lane with packed fp16 FMAs and is the A fragment
+//       of mma.m16n8k16: rows (sp, s mod 8), one M-tile per segment of eight s, K = forward colours | backward colours
+//       (lanes t = 3 pad K with zeros).  The B fragment is the link as a real 6x6 (padded 8x8) matrix, built from one
+//       32-bit load per lane.  One MMA accumulates the upper components over all directions; a second one with the
+//       forward half of B negated gives W_b h_b - W_f h_f, which sg G^dag maps onto the lower components inside the lane.
 //   5D matrices: out[s][n] = sum_s' M_hi[s][s'] X[s'][n]; the accumulator fragment is
 //       converted to fp16 (the paper's HMMA operands), transposed across the warp with movmatrix into a
 //       B fragment, and multiplied by the constant A fragment of M (host-built, one uint4 per lane and chirality).
@@ -32,13 +33,6 @@ __device__ __forceinline__ void mma16816(float (&d)[4], uint32_t a0, uint32_t a1
   asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
                : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
                : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
-}
-// k = 8 variant: A = {(row g, k 2t..2t+1), (row g+8, same k)}, B = one register.  Its A operand is an aligned register PAIR
-// of a 128-bit fragment load ((hi0, hi1) of one sp), so no register moves precede it.
-__device__ __forceinline__ void mma1688(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t b0) {
-  asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5}, {%6}, {%0,%1,%2,%3};\n"
-               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
-               : "r"(a0), "r"(a1), "r"(b0));
 }
 __device__ __forceinline__ uint32_t movmatrix_trans(uint32_t x) {
   uint32_t y;
@@ -88,43 +82,54 @@ __device__ __forceinline__ uint32_t link_bfrag(uint32_t raw, int g, int t, uint3
   return __byte_perm(w, w ^ 0x80000000u, sel);   // pad lanes: (+0, -0), harmless
 }
 
-// S += sg * gamma_mu Delta for the two M-tiles (sp = 0, 1) of one segment.  Index [sp][hi*2 + ri]; gamma matrices in
-// the chiral basis of reading R2: (g_k D)_u = -i sigma_k D_l, (g_k D)_l = +i sigma_k D_u, (g_4 D)_u = D_l, (g_4 D)_l = D_u.
-template <int MU>
-__device__ __forceinline__ void gamma_accum(float (*S)[4], const float (*D)[4], float sg) {
-  if (MU == 0) {         // u0 += -i l1, u1 += -i l0, l0 += i u1, l1 += i u0
-    S[0][0] += sg * D[1][3]; S[0][1] -= sg * D[1][2]; S[1][0] += sg * D[0][3]; S[1][1] -= sg * D[0][2];
-    S[0][2] -= sg * D[1][1]; S[0][3] += sg * D[1][0]; S[1][2] -= sg * D[0][1]; S[1][3] += sg * D[0][0];
-  } else if (MU == 1) {  // u0 -= l1, u1 += l0, l0 += u1, l1 -= u0
-    S[0][0] -= sg * D[1][2]; S[0][1] -= sg * D[1][3]; S[1][0] += sg * D[0][2]; S[1][1] += sg * D[0][3];
-    S[0][2] += sg * D[1][0]; S[0][3] += sg * D[1][1]; S[1][2] -= sg * D[0][0]; S[1][3] -= sg * D[0][1];
-  } else if (MU == 2) {  // u0 += -i l0, u1 += i l1, l0 += i u0, l1 += -i u1
-    S[0][0] += sg * D[0][3]; S[0][1] -= sg * D[0][2]; S[1][0] -= sg * D[1][3]; S[1][1] += sg * D[1][2];
-    S[0][2] -= sg * D[0][1]; S[0][3] += sg * D[0][0]; S[1][2] += sg * D[1][1]; S[1][3] -= sg * D[1][0];
-  } else {               // u += l, l += u
-    S[0][0] += sg * D[0][2]; S[0][1] += sg * D[0][3]; S[1][0] += sg * D[1][2]; S[1][1] += sg * D[1][3];
-    S[0][2] += sg * D[0][0]; S[0][3] += sg * D[0][1]; S[1][2] += sg * D[1][0]; S[1][3] += sg * D[1][1];
-  }
+// Half-spinor projection BEFORE the SU(3) product.  (1 + c gamma_mu) psi has upper part
+// h = u + c G l and lower part c G^dag h  (G = -i sigma_k, or 1 for mu = t; c = -sg forward, +sg backward), so only h (two spin
+// components) is multiplied by the link: rows of the MMA are (sp, s) and one M-tile covers a whole segment, i.e. half the MMAs
+// and half the fragment reads of a full-spinor product.  h is rounded to fp16, the MMA operand precision.
+__device__ __forceinline__ uint32_t hfma2_u32(uint32_t a, uint32_t b, uint32_t c) {
+  uint32_t d;
+  asm("fma.rn.f16x2 %0, %1, %2, %3;\n" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+  return d;
 }
-
-// One direction pair mu: S += W_f psi_f + W_b psi_b + sg gamma_mu (W_b psi_b - W_f psi_f).
-// F[2*seg + sp] / B[...] = (hi = 0, hi = 1) half2 pairs of the forward / backward neighbour: the A operand of M-tile
-// (seg, sp) is {F.x, F.y, B.x, B.y} (rows (hi, g), K = forward colours | backward colours).
+__device__ __forceinline__ uint32_t swap_h2(uint32_t x) { return __byte_perm(x, x, 0x1032); }
+struct HsConst { uint32_t P, N, Q, R; };   // half2 (sg,sg), (-sg,-sg), (sg,-sg), (-sg,sg)
+// chunk = {u0, l0, u1, l1} (half2 re,im each); fwd: c = -sg, bwd: c = +sg
+template <int MU, bool FWD>
+__device__ __forceinline__ void project_hs(const uint4& q, const HsConst& k, uint32_t& h0, uint32_t& h1) {
+  if (MU == 0)      { const uint32_t m = FWD ? k.R : k.Q; h0 = hfma2_u32(swap_h2(q.w), m, q.x); h1 = hfma2_u32(swap_h2(q.y), m, q.z); }
+  else if (MU == 1) { h0 = hfma2_u32(q.w, FWD ? k.P : k.N, q.x); h1 = hfma2_u32(q.y, FWD ? k.N : k.P, q.z); }
+  else if (MU == 2) { h0 = hfma2_u32(swap_h2(q.y), FWD ? k.R : k.Q, q.x); h1 = hfma2_u32(swap_h2(q.w), FWD ? k.Q : k.R, q.z); }
+  else              { const uint32_t m = FWD ? k.N : k.P; h0 = hfma2_u32(q.y, m, q.x); h1 = hfma2_u32(q.w, m, q.z); }
+}
+__device__ __forceinline__ void mma16816_4(float& d0, float& d1, float& d2, float& d3, uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
+  asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
+      : "+f"(d0), "+f"(d1), "+f"(d2), "+f"(d3) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+// S[2*seg + sp][hi*2 + ri]: hi = 0 accumulates W h directly; hi = 1 gets sg G^dag (W_b h_b - W_f h_f).
 template <int MU, int LS>
-__device__ __forceinline__ void hop_mu(float (&S)[MmaCfg<LS>::NMT][4], const uint2 (&F)[MmaCfg<LS>::NMT], const uint2 (&B)[MmaCfg<LS>::NMT],
-                                       uint32_t bf, uint32_t bb, float sg) {
+__device__ __forceinline__ void hop_mu_hs(float (&S)[MmaCfg<LS>::NMT][4], const uint4 (&F)[MmaCfg<LS>::NSEG], const uint4 (&B)[MmaCfg<LS>::NSEG],
+                                          uint32_t bf, uint32_t bb, float sg, const HsConst& k) {
   typedef MmaCfg<LS> Cfg;
-  float D[Cfg::NMT][4];
-#pragma unroll
-  for (int m = 0; m < Cfg::NMT; m++) { D[m][0] = D[m][1] = D[m][2] = D[m][3] = 0.f; }
   const uint32_t bfn = bf ^ 0x80008000u;
 #pragma unroll
-  for (int m = 0; m < Cfg::NMT; m++) {   // (four k = 8 MMAs per tile save the register moves but measured 10 % slower)
-    mma16816(S[m], F[m].x, F[m].y, B[m].x, B[m].y, bf, bb);
-    mma16816(D[m], F[m].x, F[m].y, B[m].x, B[m].y, bfn, bb);
+  for (int seg = 0; seg < Cfg::NSEG; seg++) {
+    uint32_t f0, f1, b0, b1;
+    project_hs<MU, true>(F[seg], k, f0, f1);
+    project_hs<MU, false>(B[seg], k, b0, b1);
+    float (&S0)[4] = S[2 * seg], (&S1)[4] = S[2 * seg + 1];
+    mma16816_4(S0[0], S0[1], S1[0], S1[1], f0, f1, b0, b1, bf, bb);
+    float d0 = 0.f, d1 = 0.f, d2 = 0.f, d3 = 0.f;   // (sp0 re, im), (sp1 re, im) of W_b h_b - W_f h_f
+    mma16816_4(d0, d1, d2, d3, f0, f1, b0, b1, bfn, bb);
+    if (MU == 0)      { S0[2] -= sg * d3; S0[3] += sg * d2; S1[2] -= sg * d1; S1[3] += sg * d0; }   // i sigma_1
+    else if (MU == 1) { S0[2] += sg * d2; S0[3] += sg * d3; S1[2] -= sg * d0; S1[3] -= sg * d1; }   // i sigma_2 = [[0,1],[-1,0]]
+    else if (MU == 2) { S0[2] -= sg * d1; S0[3] += sg * d0; S1[2] += sg * d3; S1[3] -= sg * d2; }   // i sigma_3 = diag(i,-i)
+    else              { S0[2] += sg * d0; S0[3] += sg * d1; S1[2] += sg * d2; S1[3] += sg * d3; }
   }
-#pragma unroll
-  for (int seg = 0; seg < Cfg::NSEG; seg++) gamma_accum<MU>(&S[2 * seg], &D[2 * seg], sg);
+}
+__device__ __forceinline__ uint4 lds128v(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];\n" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+  return v;
 }
 
 // X <- M X over the fifth dimension (both chiralities): X is the accumulator fragment set [seg*2+sp][hi*2+ri];
@@ -190,12 +195,6 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
                ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 
-__device__ __forceinline__ uint2 lds64(uint32_t addr) {
-  uint2 v;
-  asm volatile("ld.volatile.shared.v2.u32 {%0, %1}, [%2];\n" : "=r"(v.x), "=r"(v.y) : "r"(addr));
-  return v;
-}
-
 template <int LS> struct MmaSmem {
   enum { SLOT = LS * 48, STAGE = 8 * SLOT, WARP = 2 * STAGE + 64, BLOCK = MmaCfg<LS>::NW * WARP };   // bytes
 };
@@ -208,7 +207,7 @@ template <int LS> struct MmaSmem {
 //     site i+1 are issued before site i is computed, so a full site is always in flight per warp;
 //   * neighbour tables, link words, boundary-flip byte and the xpay operand are register-prefetched two sites ahead
 //     in two ping-pong register sets (no register is copied, so no step waits for a load it has just issued);
-//   * the A fragments are 128-bit shared-memory reads (conflict-free: a quarter warp reads 112 contiguous bytes).
+//   * the neighbour chunks are 128-bit shared-memory reads (conflict-free: a quarter warp reads 112 contiguous bytes).
 // Slots of absent neighbours (Dirichlet cut) keep stale finite data and meet a zero B fragment.
 template <int LS, int EPI, int NG>
 __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArgs<__half> a) {
@@ -222,6 +221,9 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
   int blk = blockIdx.y;
   const int stride = gridDim.x * NW;
   const float sg = (float)a.sg;
+  HsConst hsk;
+  { const uint32_t p = a.sg > 0 ? 0x3c003c00u : 0xbc00bc00u, q = a.sg > 0 ? 0xbc003c00u : 0x3c00bc00u;   // half2 (lo, hi) = (sg, sg), (sg, -sg)
+    hsk.P = p; hsk.N = p ^ 0x80008000u; hsk.Q = q; hsk.R = q ^ 0x80008000u; }
   float part = 0.f;
 
   // per-block-row base pointers (64-bit once per Dirichlet block); everything below is 32-bit offsets in units of uint4
@@ -313,16 +315,15 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
 #pragma unroll
     for (int m = 0; m < NMT; m++) { S[m][0] = S[m][1] = S[m][2] = S[m][3] = 0.f; }
     mbar_wait(bar_u32 + 8 * stg, parity);
-    // 64-bit shared-memory reads ((hi0, hi1) of one sp).  ld.volatile keeps ptxas from merging the two halves of a chunk
-    // into one 128-bit read, so that the MMA's A operand {F.x, F.y, B.x, B.y} is allocated as one register quad without moves.
+    // 128-bit shared-memory reads: the chunk {u0, l0, u1, l1} of colour t at s = g (and 8 + g), conflict free
     const uint32_t sb = stage_u32 + stg * SM::STAGE;
 #define MSPCG_HOP_MU(MU)                                                                       \
     if (have & (3u << (2 * MU))) {                                                             \
-      uint2 Ff[NMT], Bb[NMT];                                                                  \
+      uint4 Ff[NSEG], Bb[NSEG];                                                                \
       const uint32_t pf = sb + (2 * MU) * SM::SLOT, pb = pf + SM::SLOT;                        \
-      Ff[0] = lds64(pf + 16 * fo0); Bb[0] = lds64(pb + 16 * fo0); Ff[1] = lds64(pf + 16 * fo0 + 8); Bb[1] = lds64(pb + 16 * fo0 + 8); \
-      if (NSEG == 2) { Ff[NMT - 2] = lds64(pf + 16 * fo1); Bb[NMT - 2] = lds64(pb + 16 * fo1); Ff[NMT - 1] = lds64(pf + 16 * fo1 + 8); Bb[NMT - 1] = lds64(pb + 16 * fo1 + 8); } \
-      hop_mu<MU, LS>(S, Ff, Bb, bfr[2 * MU], bfr[2 * MU + 1], sg);                             \
+      Ff[0] = lds128v(pf + 16 * fo0); Bb[0] = lds128v(pb + 16 * fo0);                          \
+      if (NSEG == 2) { Ff[NSEG - 1] = lds128v(pf + 16 * fo1); Bb[NSEG - 1] = lds128v(pb + 16 * fo1); } \
+      hop_mu_hs<MU, LS>(S, Ff, Bb, bfr[2 * MU], bfr[2 * MU + 1], sg, hsk);                     \
     }
     MSPCG_HOP_MU(0) MSPCG_HOP_MU(1) MSPCG_HOP_MU(2) MSPCG_HOP_MU(3)
 #undef MSPCG_HOP_MU
