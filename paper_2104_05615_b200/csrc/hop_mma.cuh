@@ -265,7 +265,7 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
     __syncwarp();
   }
 
-  struct Meta { int nbv; uint32_t lk[8]; unsigned fl; uint4 aux[NSEG]; };
+  struct Meta { int nbv; uint32_t lk[8]; unsigned fl; };
   auto ld_meta = [&](int st, Meta& m) {
     const bool ok = st < a.n_out;
     m.nbv = (ok && lane < 8) ? __ldg(nbr + st * 8 + lane) : -1;
@@ -274,12 +274,13 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
 #pragma unroll
     for (int d = 0; d < 8; d++) m.lk[d] = (ok && lk_mine) ? __ldg(lk + d * (NG / 2)) : 0u;
   };
-  auto ld_aux = [&](int st, Meta& m) {
+  // the xpay operand of the site itself: loaded at the top of a step, consumed in its epilogue (the hop hides the latency)
+  auto ld_aux = [&](int st, uint4 (&x)[NSEG]) {
     if (EPI != EPI_PLAIN) {
-      const bool ok = st < a.n_out && st < a.n_aux;
+      const bool ok = st < a.n_aux;
       const uint4* p = aux4 + st * (LS * 3);
-      m.aux[0] = (ok && st0) ? __ldg(p + fo0) : make_uint4(0, 0, 0, 0);
-      if (NSEG == 2) m.aux[NSEG - 1] = (ok && st1) ? __ldg(p + fo1) : make_uint4(0, 0, 0, 0);
+      x[0] = (ok && st0) ? __ldg(p + fo0) : make_uint4(0, 0, 0, 0);
+      if (NSEG == 2) x[NSEG - 1] = (ok && st1) ? __ldg(p + fo1) : make_uint4(0, 0, 0, 0);
     }
   };
   // issue the eight neighbour copies of the site whose table is m.nbv into stage `stg`
@@ -294,7 +295,8 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
 
   auto step = [&](int site, int stg, uint32_t parity, Meta& cur, const Meta& nxt) {
     const int far = site + 2 * stride;
-    uint4 dv[NSEG];
+    uint4 dv[NSEG], av[NSEG];
+    ld_aux(site, av);
     if (EPI == EPI_XPAY && dot4 != nullptr) {
       const uint4* p = dot4 + site * (LS * 3);
       dv[0] = st0 ? __ldg(p + fo0) : make_uint4(0, 0, 0, 0);
@@ -339,8 +341,7 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
       if (NSEG == 2) { if (st1) po[fo1] = o[NSEG - 1]; }
     } else {
       float V[NMT][4];
-      frag_to_float<LS>(cur.aux, V);
-      ld_aux(far, cur);
+      frag_to_float<LS>(av, V);
 #pragma unroll
       for (int m = 0; m < NMT; m++) {
 #pragma unroll
@@ -382,7 +383,6 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
     part = 0.f;
     Meta mA, mB;
     ld_meta(site0, mA); ld_meta(site0 + stride, mB);
-    ld_aux(site0, mA); ld_aux(site0 + stride, mB);
     issue(mA, 0);
     int nst = 0;
     for (int site = site0; site < a.n_out; site += 2 * stride) {
