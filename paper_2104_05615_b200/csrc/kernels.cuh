@@ -650,12 +650,16 @@ template <typename T> __device__ __forceinline__ void stchunk(T* base, long i, c
   typedef typename ST<T>::V V; V q; packV(q, v); reinterpret_cast<V*>(base)[i] = q;
 }
 
-// Outer-iteration BLAS-1 (Algorithm 1): x += alpha p, r -= alpha Ap, out[0] += |r|^2.
+// Outer-iteration BLAS-1 (Algorithm 1): alpha = <r,z> / <p,Ap> with <p,Ap> read from device memory (no host
+// round trip between the operator and this kernel; alpha = 0 if <p,Ap> <= 0, the host reports the breakdown),
+// x += alpha p, r -= alpha Ap, out[0] += |r|^2.
 template <typename T>
 __global__ void k_outer_update(const T* __restrict__ p, const T* __restrict__ q, T* __restrict__ r, T* __restrict__ x,
-                               long nchunk, double alpha, double* out) {
+                               long nchunk, double rz, const double* __restrict__ pAp, double* out) {
   __shared__ double red[32];
   constexpr int PER = ST<T>::PER;
+  const double pq = *pAp;
+  const double alpha = pq > 0.0 ? rz / pq : 0.0;
   const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
   double part = 0;
   if (i < nchunk) {

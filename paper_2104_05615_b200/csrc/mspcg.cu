@@ -707,14 +707,13 @@ int solve_impl(mspcg_ctx* c, const double* b_abi, double* x_abi, const mspcg_sol
       SOLVE_CUDA(sc_zero(c, 4, st));
       SOLVE_CUDA(normal_full<TS>(c, obS, p, Ap, mp, c->sc, st));
       stt->outer_applies++;
-      SOLVE_CUDA(sc_read(c, 1, st));
-      const double pAp = c->sc_host[0];
-      if (!(pAp > 0.0)) { stt->breakdown = 1; rc = MSPCG_EBREAKDOWN; break; }
-      alpha = rz / pAp;                                       // alpha_k = <r_k,z_k>/<p_k,A p_k>
-      { const long nchunk = nreal / ST<TS>::PER;
-        k_outer_update<TS><<<(unsigned)((nchunk + 255) / 256), 256, 0, st>>>(p, Ap, rlo, xlo, nchunk, alpha, c->sc + 1);
+      { const long nchunk = nreal / ST<TS>::PER;              // alpha_k = <r_k,z_k>/<p_k,A p_k> is formed on the device
+        k_outer_update<TS><<<(unsigned)((nchunk + 255) / 256), 256, 0, st>>>(p, Ap, rlo, xlo, nchunk, rz, c->sc, c->sc + 1);
         c->launches++; }
       SOLVE_CUDA(sc_read(c, 2, st));
+      const double pAp = c->sc_host[0];
+      if (!(pAp > 0.0)) { stt->breakdown = 1; rc = MSPCG_EBREAKDOWN; break; }   // the update kernel used alpha = 0
+      alpha = rz / pAp;
       rnorm = std::sqrt(c->sc_host[1]) * sigma;
       k++;
       if (prm->history && k <= prm->history_len) prm->history[k - 1] = rnorm / bnorm;
