@@ -51,6 +51,8 @@ def stage_sites(geo, full):
 def flops_normal(st, Ls):
     """Flops of one D^dag D (or A_s, all blocks) application; SURVEY 8(d) convention."""
     hop, bid, xpay, dense = 1320, 72, 48, 48 * Ls
+    # (SURVEY 8(d) convention: kernel 3 counts two contractions and the xpay on every site of its list, although the library
+    # applies the product matrix M5^-dag M5^-1 as one contraction on the halo sites of a Dirichlet block)
     per_block = (bid * st["nE0"] + (hop + dense) * st["nO"] + (hop + 2 * dense + xpay) * st["nE"]
                  + (hop + dense) * st["nO"] + (hop + bid + xpay) * st["nE0"]) * Ls
     return per_block * st["nblk"]

@@ -40,10 +40,10 @@ struct Arena {
 struct GeomDev { int *nbrE = nullptr, *nbrO = nullptr; short *cE = nullptr, *cO = nullptr, *origin = nullptr; };
 
 // One set of fifth-dimension matrices (device, transposed per chirality: m[ch][s'][s]) in one compute type.
-template <typename C> struct MatSet { C *K2 = nullptr, *K3a = nullptr, *K3b = nullptr, *K4 = nullptr, *K5 = nullptr; };
+template <typename C> struct MatSet { C *K2 = nullptr, *K3a = nullptr, *K3b = nullptr, *K4 = nullptr, *K5 = nullptr, *K3h = nullptr; };
 // The same matrices as fp16 mma.m16n8k16 A fragments [chirality 2][lane 32] (hop_mma.cuh).
-struct MatFrag { uint4 *K2 = nullptr, *K3a = nullptr, *K3b = nullptr, *K4 = nullptr, *K5 = nullptr; };
-struct HostMats { std::vector<double> K2, K3a, K3b, K4, K5; Mat A, F, Ainv; double diag, off; };
+struct MatFrag { uint4 *K2 = nullptr, *K3a = nullptr, *K3b = nullptr, *K4 = nullptr, *K5 = nullptr, *K3h = nullptr; };
+struct HostMats { std::vector<double> K2, K3a, K3b, K4, K5, K3h; Mat A, F, Ainv; double diag, off; };
 
 // Everything one precision needs to apply D^dag D on one geometry.
 struct OpBuf {
@@ -123,6 +123,8 @@ bool build_host_mats(HostMats& h, int Ls, double b, double c, double M5, double 
   transposed(At, h.Ainv, h.K3b);                               // M5^-dag              (kernel 3, second factor)
   transposed(mat_mul(At, Ft), mat_mul(h.Ainv, h.F), h.K4);     // M5^-dag Mphi^dag     (kernel 4)
   transposed(Ft, h.F, h.K5);                                   // Mphi^dag             (kernel 5)
+  transposed(mat_mul(At, h.Ainv), mat_mul(h.Ainv, At), h.K3h); // - M5^-dag M5^-1      (kernel 3 on the halo sites of a Dirichlet block,
+  for (double& v : h.K3h) v = -v;                              //                       where the xpay operand is zero: w = -M5^-dag M5^-1 D^w tO)
   return true;
 }
 
@@ -133,10 +135,10 @@ void carve_geom(Arena& a, GeomDev& g, const Geometry& h) {
 }
 template <typename C> void carve_mats(Arena& a, MatSet<C>& m, int Ls) {
   size_t n = (size_t)2 * Ls * Ls;
-  m.K2 = a.take<C>(n); m.K3a = a.take<C>(n); m.K3b = a.take<C>(n); m.K4 = a.take<C>(n); m.K5 = a.take<C>(n);
+  m.K2 = a.take<C>(n); m.K3a = a.take<C>(n); m.K3b = a.take<C>(n); m.K4 = a.take<C>(n); m.K5 = a.take<C>(n); m.K3h = a.take<C>(n);
 }
 void carve_frags(Arena& a, MatFrag& m) {
-  m.K2 = a.take<uint4>(64); m.K3a = a.take<uint4>(64); m.K3b = a.take<uint4>(64); m.K4 = a.take<uint4>(64); m.K5 = a.take<uint4>(64);
+  m.K2 = a.take<uint4>(64); m.K3a = a.take<uint4>(64); m.K3b = a.take<uint4>(64); m.K4 = a.take<uint4>(64); m.K5 = a.take<uint4>(64); m.K3h = a.take<uint4>(64);
 }
 void carve_links(Arena& a, OpBuf& o, const Geometry& g, int prec, int ng) {
   o.prec = prec; o.ng = ng; o.have = true;
@@ -214,7 +216,9 @@ template <typename T, int LS, int EPI> size_t hop_smem() {
   return sizeof(C) * ((size_t)SM::NS * SM::USTRIDE + (size_t)SM::NS * SM::SSTRIDE + (size_t)(EPI == EPI_K3 ? 4 : 2) * LS * LS) + sizeof(int) * SM::NS * 8;
 }
 template <typename T, int LS, int EPI>
-cudaError_t launch_hop(mspcg_ctx* c, const HopArgs<T>& a, int nblk, cudaStream_t st) {
+cudaError_t launch_hop(mspcg_ctx* c, const HopArgs<T>& a, int nblk, cudaStream_t st, bool timed = true) {
+  const bool was_timing = c->timing;
+  if (!timed) c->timing = false;   // the caller times a group of launches as one (kernel 3 = interior + halo launch)
   const int kind = EPI == EPI_PLAIN ? KIND_HOP_PLAIN : (EPI == EPI_K3 ? KIND_HOP_K3 : KIND_HOP_XPAY);
   if constexpr (std::is_same<T, __half>::value) {   // fp16 storage: warp-per-site tensor-core kernel (hop_mma.cuh)
     constexpr int NW = MmaCfg<LS>::NW;
@@ -243,6 +247,7 @@ cudaError_t launch_hop(mspcg_ctx* c, const HopArgs<T>& a, int nblk, cudaStream_t
     { TimedLaunch tl(c, kind, st); k_hop<T, LS, EPI><<<grid, block, sm, st>>>(a); }
   }
   c->launches++;
+  c->timing = was_timing;
   return cudaPeekAtLastError();
 }
 template <typename T, int LS>
@@ -305,11 +310,24 @@ cudaError_t apply_normal(mspcg_ctx* c, const OpView<T>& v, MphiArgs<T> mp, const
   a.in = v.t1; a.in_stride = v.nE0; a.n_in_limit = v.nE0; a.out = v.tO; a.out_stride = v.nO; a.n_out = v.nO;
   a.nbr = v.nbrO; a.links = v.linksO; a.flip = v.flipO; a.link_stride = v.nO; a.mat1 = m.K2; a.frag1 = mf.K2; a.sg = (C)1;
   if ((e = launch_hop<T, LS, EPI_PLAIN>(c, a, v.nblk, st)) != cudaSuccess) return e;
-  // K3
-  a.in = v.tO; a.in_stride = v.nO; a.n_in_limit = v.nO; a.out = v.w; a.out_stride = v.nE; a.n_out = v.nE;
+  // K3: on the interior sites (d = 0) y = p - M5^-1 D^w tO, w = M5^-dag y; on the halo sites of a Dirichlet block p = 0 and y is
+  // not needed, so w = -(M5^-dag M5^-1) D^w tO is one contraction with the product matrix (a plain-epilogue launch on the site
+  // range [nE0, nE)).  The two launches are timed as one kernel 3.
+  a.in = v.tO; a.in_stride = v.nO; a.n_in_limit = v.nO; a.out = v.w; a.out_stride = v.nE; a.n_out = v.nE0;
   a.out2 = v.y; a.out2_stride = v.nE0; a.n_out2 = v.nE0; a.aux = p; a.aux_stride = v.nE0; a.n_aux = v.nE0;
   a.nbr = v.nbrE; a.links = v.linksE; a.flip = v.flipE; a.link_stride = v.nE; a.mat1 = m.K3a; a.mat2 = m.K3b; a.frag1 = mf.K3a; a.frag2 = mf.K3b;
-  if ((e = launch_hop<T, LS, EPI_K3>(c, a, v.nblk, st)) != cudaSuccess) return e;
+  {
+    TimedLaunch tl(c, KIND_HOP_K3, st);
+    if ((e = launch_hop<T, LS, EPI_K3>(c, a, v.nblk, st, false)) != cudaSuccess) return e;
+    if (v.nE > v.nE0) {
+      HopArgs<T> h = a;
+      h.out = v.w + (size_t)v.nE0 * LS * 24; h.n_out = v.nE - v.nE0;
+      h.out2 = nullptr; h.n_out2 = 0; h.aux = nullptr; h.n_aux = 0;
+      h.nbr = v.nbrE + (size_t)v.nE0 * 8; h.links = v.linksE + (size_t)v.nE0 * 8 * v.ng; h.flip = v.flipE + v.nE0;
+      h.mat1 = m.K3h; h.mat2 = nullptr; h.frag1 = mf.K3h; h.frag2 = nullptr;
+      if ((e = launch_hop<T, LS, EPI_PLAIN>(c, h, v.nblk, st, false)) != cudaSuccess) return e;
+    }
+  }
   // K4
   a.in = v.w; a.in_stride = v.nE; a.n_in_limit = v.nE; a.out = v.tO; a.out_stride = v.nO; a.n_out = v.nO;
   a.out2 = nullptr; a.aux = nullptr; a.n_aux = 0; a.nbr = v.nbrO; a.links = v.linksO; a.flip = v.flipO; a.link_stride = v.nO;
@@ -482,9 +500,9 @@ cudaError_t build_links_any(mspcg_ctx* c, const double* U, OpBuf& o, const Geome
 }
 
 template <typename C> cudaError_t upload_mats(const MatSet<C>& m, const HostMats& h, cudaStream_t st) {
-  const std::vector<double>* src[5] = {&h.K2, &h.K3a, &h.K3b, &h.K4, &h.K5};
-  C* dst[5] = {m.K2, m.K3a, m.K3b, m.K4, m.K5};
-  for (int i = 0; i < 5; i++) {
+  const std::vector<double>* src[6] = {&h.K2, &h.K3a, &h.K3b, &h.K4, &h.K5, &h.K3h};
+  C* dst[6] = {m.K2, m.K3a, m.K3b, m.K4, m.K5, m.K3h};
+  for (int i = 0; i < 6; i++) {
     std::vector<C> tmp(src[i]->begin(), src[i]->end());
     cudaError_t e = cudaMemcpyAsync(dst[i], tmp.data(), tmp.size() * sizeof(C), cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return e;
@@ -495,9 +513,9 @@ template <typename C> cudaError_t upload_mats(const MatSet<C>& m, const HostMats
 // fp16 A fragments of mma.m16n8k16 (row-major 16x16, zero padded) of the five matrices; src is the transposed-per-
 // chirality array of build_host_mats: M_ch[s][s'] = src[(ch*n + s')*n + s].
 cudaError_t upload_frags(const MatFrag& m, const HostMats& h, int n, cudaStream_t st) {
-  const std::vector<double>* src[5] = {&h.K2, &h.K3a, &h.K3b, &h.K4, &h.K5};
-  uint4* dst[5] = {m.K2, m.K3a, m.K3b, m.K4, m.K5};
-  for (int i = 0; i < 5; i++) {
+  const std::vector<double>* src[6] = {&h.K2, &h.K3a, &h.K3b, &h.K4, &h.K5, &h.K3h};
+  uint4* dst[6] = {m.K2, m.K3a, m.K3b, m.K4, m.K5, m.K3h};
+  for (int i = 0; i < 6; i++) {
     std::vector<uint32_t> tmp(2 * 32 * 4);
     auto M = [&](int ch, int s, int sp) -> float { return (s < n && sp < n) ? (float)(*src[i])[((size_t)ch * n + sp) * n + s] : 0.f; };
     auto h2 = [&](float lo, float hi) -> uint32_t {
