@@ -92,6 +92,17 @@ def test_MdagM_low_precision(prec, tol, recon):
     assert rel(out, ref) <= tol
 
 
+@pytest.mark.parametrize("dims,Ls,block", [((4, 4, 4, 8), 4, (2, 2, 4, 4)), ((4, 4, 6, 4), 6, (2, 2, 2, 2)),
+                                           ((8, 4, 4, 8), 12, (4, 4, 2, 4)), ((4, 8, 4, 8), 16, (4, 4, 4, 4))])
+def test_fp16_tensor_core_hop_every_compiled_Ls(dims, Ls, block):
+    """The fp16 path (half-spinor projection, SU(3) and Ls x Ls contractions on the tensor cores) at every compiled Ls: one and
+    two row segments, partially filled second segment (Ls = 12), full lattice and Dirichlet blocks."""
+    ora, g, torch = setup(dims, Ls, 0.02, block, outer=F16, inner=F16)
+    v = synth.gaussian_spinor_abi(dims, Ls, 19)
+    assert rel(g.apply_MdagM(dev(torch, v), F16).cpu().numpy(), ora.apply_MdagM(v)) <= 2e-3
+    assert rel(g.apply_precond(dev(torch, v), 6, F64).cpu().numpy(), ora.apply_precond(v, 6)) <= 2e-2
+
+
 @pytest.mark.parametrize("dims,Ls,block", GEOMS)
 def test_A_block_fp64(dims, Ls, block):
     ora, g, torch = setup(dims, Ls, 0.02, block)
