@@ -133,13 +133,13 @@ __device__ __forceinline__ uint4 lds128v(uint32_t addr) {
 }
 
 // X <- M X over the fifth dimension (both chiralities): X is the accumulator fragment set [seg*2+sp][hi*2+ri];
-// mfrag[hi*32 + lane] is the A fragment of the 16x16 zero-padded matrix of chirality hi.
+// mfrag[hi*32 + lane] is the A fragment of the 16x16 zero-padded matrix of chirality hi (shared-memory copy).
 template <int LS>
 __device__ __forceinline__ void dense5d_mma(float (&X)[MmaCfg<LS>::NMT][4], const uint4* __restrict__ mfrag, int lane) {
   typedef MmaCfg<LS> Cfg;
 #pragma unroll
   for (int hi = 0; hi < 2; hi++) {
-    const uint4 A = __ldg(mfrag + hi * 32 + lane);
+    const uint4 A = mfrag[hi * 32 + lane];
 #pragma unroll
     for (int sp = 0; sp < 2; sp++) {
       const uint32_t b0 = movmatrix_trans(pack_h2(X[sp][2 * hi], X[sp][2 * hi + 1]));
@@ -216,6 +216,10 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
   constexpr int NSEG = Cfg::NSEG, NMT = Cfg::NMT, NW = Cfg::NW;
   extern __shared__ __align__(128) unsigned char smraw[];
   __shared__ double red[NW];
+  __shared__ uint4 sfrag[(EPI == EPI_K3 ? 2 : 1) * 64];   // A fragments of the 5D matrices, fetched once per thread block
+  if (threadIdx.x < 64) sfrag[threadIdx.x] = __ldg(a.frag1 + threadIdx.x);
+  if (EPI == EPI_K3) { if (threadIdx.x >= 64) sfrag[threadIdx.x] = __ldg(a.frag2 + threadIdx.x - 64); }
+  __syncthreads();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int g = lane >> 2, t = lane & 3;
   int blk = blockIdx.y;
@@ -331,7 +335,7 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
 #undef MSPCG_HOP_MU
     __syncwarp();                              // the stage may be overwritten by the copies issued in the next step
 
-    dense5d_mma<LS>(S, a.frag1, lane);
+    dense5d_mma<LS>(S, sfrag, lane);
 
     uint4 o[NSEG];
     uint4* po = out4 + site * (LS * 3);
@@ -354,7 +358,7 @@ __global__ void __launch_bounds__(32 * MmaCfg<LS>::NW, 4) k_hop_mma(const HopArg
           if (st0) p2[fo0] = o[0];
           if (NSEG == 2) { if (st1) p2[fo1] = o[NSEG - 1]; }
         }
-        dense5d_mma<LS>(S, a.frag2, lane);
+        dense5d_mma<LS>(S, sfrag + 64, lane);
         float_to_frag<LS>(S, o);
       }
       if (st0) po[fo0] = o[0];
