@@ -403,6 +403,23 @@ def extras(torch, g, cfg, U, src, d_src, geo, peak, args):
     g2.configure(F16, F64, 18)
     g2.load_gauge(U, -1)
     ex["DdagD_fp16"] = time_op(g2, F16, 2)
+    if Ls in (8, 12, 16):
+        # the dense 5D contraction M5^-1 on its own as a tcgen05 GEMM (mspcg_apply_M5inv): four buffer pairs in rotation
+        # (one fp16 vector pair is smaller than L2), flops by the minimal count 48*Ls per 5D site and as issued (8x: delta_jj' zeros)
+        ins = [g2.pack(d_src, F16) for _ in range(4)]
+        outs = [g2.new_native(F16) for _ in range(4)]
+        cnt = [0]
+
+        def m5():
+            g2.apply_M5inv(ins[cnt[0] & 3], False, out=outs[cnt[0] & 3])
+            cnt[0] += 1
+        ms = timed(torch, m5, 4 * steps, 4 * warm) / (4 * steps)
+        n5 = ins[0].numel() * ins[0].element_size() // 48
+        e = op_entry(ms, 48.0 * Ls * n5, 2.0 * 48 * n5)
+        e["GFLOPs_issued_on_tensor_cores"] = 8 * e["GFLOPs"]
+        e["note"] = "tcgen05.mma kind::f16, fp32 accumulation in TMEM; 4 buffer pairs rotated"
+        ex["M5inv_tcgen05_fp16"] = e
+        del ins, outs
     ex["Mpre_k%d_fp64" % k] = time_pre(g2, F64, 8, 8)
     g2.close()
     torch.cuda.empty_cache()

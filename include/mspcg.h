@@ -72,6 +72,15 @@ size_t mspcg_vec_bytes(const mspcg_ctx* ctx, int prec);
 int mspcg_pack(mspcg_ctx* ctx, const double* abi_dev, void* native_dev, int prec, void* stream);
 int mspcg_unpack(mspcg_ctx* ctx, const void* native_dev, double* abi_dev, int prec, void* stream);
 
+/* out = M5^-1 in (dagger = 0) or M5^-dag in (dagger != 0) on an fp16 NATIVE one-parity vector (mspcg_pack with MSPCG_F16):
+ * the dense fifth-dimension contraction of PAPER.md:260-264 (an Ls x Ls real matrix per chirality times the Ls x 24*sites
+ * panel; M5^-1 of eq. 4-5, closed form R4) as a stand-alone tcgen05.mma GEMM with fp16 operands and fp32
+ * accumulation in tensor memory.  Inside mspcg_apply_MdagM / mspcg_apply_precond the same contraction is fused into the
+ * hop kernels; this entry point applies it on its own.  Ls must be 8, 12 or 16.  in_dev, out_dev: DEVICE, caller-owned,
+ * mspcg_vec_bytes(ctx, MSPCG_F16) bytes each, must not alias.  Needs the workspace, not the gauge field.  Asynchronous
+ * on `stream`.  Errors: ENOWORKSPACE, EINVAL, ECUDA. */
+int mspcg_apply_M5inv(mspcg_ctx* ctx, const void* in_dev, void* out_dev, int dagger, void* stream);
+
 /* out = D^dag D in  on the whole periodic/antiperiodic lattice (eq. 9-10, 230-258 eq. 15-16:
  * one Mphi kernel and four fused hop kernels).  prec = MSPCG_F64 or the configured outer_prec.
  * layout ABI: in/out are fp64 ABI vectors (converted on entry/exit); NATIVE: vectors of `prec` from mspcg_pack.

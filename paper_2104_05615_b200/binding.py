@@ -24,7 +24,7 @@ SYMBOLS = [
     "mspcg_unpack", "mspcg_apply_MdagM", "mspcg_apply_precond", "mspcg_apply_MdagM_host",
     "mspcg_apply_precond_host", "mspcg_apply_A_block", "mspcg_set_reduced_ls", "mspcg_solve", "mspcg_launch_count",
     "mspcg_timing", "mspcg_timing_read", "mspcg_update_T", "mspcg_train_eval", "mspcg_train_T",
-    "mspcg_prepare_source", "mspcg_reconstruct_odd", "mspcg_apply_full",
+    "mspcg_prepare_source", "mspcg_reconstruct_odd", "mspcg_apply_full", "mspcg_apply_M5inv",
 ]
 
 
@@ -66,6 +66,7 @@ def load_library():
     L.mspcg_pack.argtypes = [vp, vp, vp, i, vp]
     L.mspcg_unpack.argtypes = [vp, vp, vp, i, vp]
     L.mspcg_apply_MdagM.argtypes = [vp, vp, vp, i, i, vp]
+    L.mspcg_apply_M5inv.argtypes = [vp, vp, vp, i, vp]
     L.mspcg_apply_precond.argtypes = [vp, vp, vp, i, i, i, i, vp]
     L.mspcg_apply_MdagM_host.argtypes = [vp, vp, vp, i]
     L.mspcg_apply_precond_host.argtypes = [vp, vp, vp, i, i, i]
@@ -230,6 +231,12 @@ class Mspcg:
         torch = _torch()
         out = torch.empty_like(v) if out is None else out
         self._check(self.lib.mspcg_apply_MdagM(self.h, C.c_void_p(v.data_ptr()), C.c_void_p(out.data_ptr()), prec, layout, self._stream()))
+        return out
+
+    def apply_M5inv(self, v_native_f16, dagger=False, out=None):
+        torch = _torch()
+        out = torch.empty_like(v_native_f16) if out is None else out
+        self._check(self.lib.mspcg_apply_M5inv(self.h, C.c_void_p(v_native_f16.data_ptr()), C.c_void_p(out.data_ptr()), int(bool(dagger)), self._stream()))
         return out
 
     def apply_precond(self, r, n_inner, io_prec=F64, layout=LAYOUT_ABI, out=None, use_reduced=0):

@@ -81,6 +81,7 @@ struct mspcg_ctx {
   double *rho = nullptr, *pq = nullptr; float* scale = nullptr; double* sc = nullptr;  // device scalars
   double* Tm = nullptr;          // device copy of the reduced-Ls transfer matrix T_host (A10)
   double* Gdev = nullptr;        // gradient accumulator of the T training (A12)
+  __half* Bm5[2] = {nullptr, nullptr};       // fp16 B-operand images of M5^-1 and M5^-dag for k_dense5d_tc
   __half *Bfwd = nullptr, *Bbwd = nullptr;   // fp16 B-operand images of T and T^dag for the tcgen05 transfer kernels
   bool transfer_tc = true;       // use them when (Ls, Ls_hat) is a compiled pair and the inner storage is fp16
   double* sc_host = nullptr;     // pinned
@@ -163,6 +164,7 @@ void carve(mspcg_ctx* c, Arena& a) {
   c->e_int_to_cb = a.take<int>(L.e_int_to_cb.size()); c->o_int_to_cb = a.take<int>(L.o_int_to_cb.size());
   c->negI = a.take<double>((size_t)2 * c->Ls * c->Ls);
   carve_mats(a, c->md, c->Ls); carve_mats(a, c->mf32, c->Ls); carve_frags(a, c->mfr);
+  for (int d = 0; d < 2; d++) c->Bm5[d] = a.take<__half>((size_t)64 * c->Ls * c->Ls);
   if (c->Ls_hat) { carve_mats(a, c->md_hat, c->Ls_hat); carve_mats(a, c->mf32_hat, c->Ls_hat); carve_frags(a, c->mfr_hat); }
   c->rho = a.take<double>((size_t)(KMAX + 1) * L.nblk); c->pq = a.take<double>((size_t)KMAX * L.nblk);
   c->scale = a.take<float>(L.nblk); c->sc = a.take<double>(16);
@@ -537,6 +539,25 @@ cudaError_t upload_frags(const MatFrag& m, const HostMats& h, int n, cudaStream_
 }
 template <typename V> cudaError_t up(void* dst, const std::vector<V>& src, cudaStream_t st) {
   return cudaMemcpyAsync(dst, src.data(), src.size() * sizeof(V), cudaMemcpyHostToDevice, st);
+}
+
+// fp16 B-operand images of M5^-1 (d = 0) and M5^-dag (d = 1) for k_dense5d_tc: B[n = (s, j)][k = (s', j')] = M_hi[s][s'] delta_jj',
+// j = (sp, hi, re/im), hi = (j >> 1) & 1; on P+ (hi = 0) M5^-1 is A+^-1 (hm.Ainv), on P- its transpose (R3); the dagger swaps them.
+// Same canonical K-major layout as the T images below.
+int upload_m5_images(mspcg_ctx* ctx, cudaStream_t st) {
+  const int Ls = ctx->Ls;
+  for (int d = 0; d < 2; d++) {
+    std::vector<__half> img((size_t)64 * Ls * Ls, __float2half_rn(0.f));
+    for (int s = 0; s < Ls; s++) for (int sp = 0; sp < Ls; sp++) for (int j = 0; j < 8; j++) {
+      const int hi = (j >> 1) & 1;
+      const double v = ((hi ^ d) == 0) ? ctx->hm.Ainv.at(s, sp) : ctx->hm.Ainv.at(sp, s);
+      const int n = s * 8 + j, k = sp * 8 + j;
+      img[(size_t)(n / 8) * Ls * 64 + (size_t)(k / 8) * 64 + (n % 8) * 8 + (k % 8)] = __float2half_rn((float)v);
+    }
+    CUDA_OK(ctx, cudaMemcpyAsync(ctx->Bm5[d], img.data(), img.size() * sizeof(__half), cudaMemcpyHostToDevice, st));
+    CUDA_OK(ctx, cudaStreamSynchronize(st));
+  }
+  return MSPCG_OK;
 }
 
 // Device copies of the reduced-Ls transfer matrix: fp64 T for the generic kernels and the fp16 B-operand images of T and
@@ -956,6 +977,7 @@ int mspcg_set_workspace(mspcg_ctx* ctx, void* workspace_dev, size_t bytes, void*
   CUDA_OK(ctx, cudaStreamSynchronize(st));
   CUDA_OK(ctx, upload_mats<double>(ctx->md, ctx->hm, st)); CUDA_OK(ctx, upload_mats<float>(ctx->mf32, ctx->hm, st));
   CUDA_OK(ctx, upload_frags(ctx->mfr, ctx->hm, ctx->Ls, st));
+  { int rc_ = upload_m5_images(ctx, st); if (rc_) return rc_; }
   if (ctx->Ls_hat) {
     CUDA_OK(ctx, upload_mats<double>(ctx->md_hat, ctx->hm_hat, st)); CUDA_OK(ctx, upload_mats<float>(ctx->mf32_hat, ctx->hm_hat, st));
     CUDA_OK(ctx, upload_frags(ctx->mfr_hat, ctx->hm_hat, ctx->Ls_hat, st));
@@ -992,6 +1014,28 @@ int mspcg_unpack(mspcg_ctx* ctx, const void* native_dev, double* abi_dev, int pr
   if (!abi_dev || !native_dev || !prec_ok(prec)) return fail(ctx, MSPCG_EINVAL, "bad argument");
   CUDA_OK(ctx, pack_any(ctx, abi_dev, const_cast<void*>(native_dev), prec, 0, (cudaStream_t)stream));
   return MSPCG_OK;
+}
+
+int mspcg_apply_M5inv(mspcg_ctx* ctx, const void* in_dev, void* out_dev, int dagger, void* stream) {
+  int rc = check_ready(ctx, false); if (rc) return rc;
+  if (!in_dev || !out_dev || in_dev == out_dev) return fail(ctx, MSPCG_EINVAL, "bad pointer or aliasing");
+  cudaStream_t st = (cudaStream_t)stream;
+  Dense5dTcArgs a;
+  a.in = reinterpret_cast<const uint4*>(in_dev); a.out = reinterpret_cast<uint4*>(out_dev);
+  a.Bimg = ctx->Bm5[dagger ? 1 : 0]; a.n_sites = (long)(v5h(ctx, ctx->Ls) / ctx->Ls);
+  const unsigned grid = (unsigned)((a.n_sites + tc::TILE - 1) / tc::TILE);
+#define DT(LSV)                                                                                                          \
+  if (ctx->Ls == LSV) {                                                                                                  \
+    static bool attr = false;                                                                                            \
+    if (!attr) { cudaFuncSetAttribute(k_dense5d_tc<LSV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Dense5dTcCfg<LSV>::SMEM); attr = true; } \
+    k_dense5d_tc<LSV><<<grid, 128, Dense5dTcCfg<LSV>::SMEM, st>>>(a);                                                \
+    ctx->launches++;                                                                                                     \
+    CUDA_OK(ctx, cudaPeekAtLastError());                                                                                 \
+    return MSPCG_OK;                                                                                                     \
+  }
+  DT(8) DT(12) DT(16)
+#undef DT
+  return fail(ctx, MSPCG_EINVAL, "mspcg_apply_M5inv: Ls must be 8, 12 or 16");
 }
 
 int mspcg_apply_MdagM(mspcg_ctx* ctx, const void* in_dev, void* out_dev, int prec, int layout, void* stream) {

@@ -256,4 +256,87 @@ __global__ void __launch_bounds__(128, 1) k_reduce_end_tc(const TransferArgs a) 
   if (warp == 0) tc::tmem_free<Cfg::TMEM_COLS>(tmem);
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// The dense fifth-dimension contraction M5^-1 / M5^-dag as a stand-alone tcgen05 GEMM (
+// north_star item 2): out[s][n] = sum_s' M_hi[s][s'] in[s'][n] on an fp16 NATIVE vector (layout of hop_mma.cuh:
+// v[site][s][colour][sp][hi][re,im]).  Per colour it is the GEMM  D[site][n] = sum_k A[site][k] B[n][k]  with
+// k = (s', j), n = (s, j), j = (sp, hi, re/im) the eight halves of one 16-byte chunk, and B[n][k] = M_hi[s][s'] delta_jj'
+// (host image, real).  The 16-byte chunk of one (site, s', colour) in HBM IS one core-matrix row of the K-major
+// canonical layout, so the A tile is filled with plain 128-bit copies, no conversion.  M = 128 sites per thread block,
+// N = K = 8 Ls, an N-column fp32 accumulator in tensor memory; the MMA does 8x the minimal flop count
+// (the delta_jj' zeros), which the tensor pipe does not notice at this size.
+// Inside the fused hop kernels the same contraction runs on register fragments (mma.sync, hop_mma.cuh); this kernel
+// serves the places where M5^-1 stands alone on an fp16 vector.
+struct Dense5dTcArgs {
+  const uint4* in; uint4* out;   // NATIVE fp16 vectors, n_sites site columns of Ls*3 chunks
+  const __half* Bimg;            // B operand image [N/8][K/8][8][8]
+  long n_sites;
+};
+template <int LS> struct Dense5dTcCfg {
+  enum { N = 8 * LS, TMEM_COLS = (N <= 32 ? 32 : (N <= 64 ? 64 : (N <= 128 ? 128 : 256))),
+         SMEM = TransferCfg<LS, LS>::A_COLOUR + TransferCfg<LS, LS>::B_BYTES + 64 };
+};
+// One thread block = 128 sites; the three colours are processed one after the other through ONE A tile and ONE accumulator
+// (36 KB + 32 KB of shared memory and N of the 512 tensor-memory columns at Ls = 16), so that three thread blocks are resident
+// per SM and the load / MMA / write-back phases of different thread blocks overlap.
+template <int LS>
+__global__ void __launch_bounds__(128, 3) k_dense5d_tc(const Dense5dTcArgs a) {
+  typedef TransferCfg<LS, LS> Cfg;
+  typedef Dense5dTcCfg<LS> DC;
+  extern __shared__ __align__(128) unsigned char tsm[];
+  __shared__ uint32_t tmem_slot;
+  unsigned char* As = tsm;
+  unsigned char* Bs = tsm + Cfg::A_COLOUR;
+  const uint32_t bar = (uint32_t)__cvta_generic_to_shared(tsm + Cfg::A_COLOUR + Cfg::B_BYTES);
+  const int tid = threadIdx.x, warp = tid >> 5;
+  const long site0 = (long)blockIdx.x * tc::TILE;
+
+  if (warp == 0) tc::tmem_alloc<DC::TMEM_COLS>(&tmem_slot);
+  if (tid == 0) { mbar_init(bar, 1); asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory"); }
+  for (int i = tid; i < Cfg::B_BYTES / 16; i += 128) reinterpret_cast<uint4*>(Bs)[i] = __ldg(reinterpret_cast<const uint4*>(a.Bimg) + i);
+  const long site = site0 + tid;                     // epilogue: thread = TMEM lane = site row
+  uint4* out4 = a.out + site * (LS * 3);
+#pragma unroll 1
+  for (int c = 0; c < 3; c++) {
+    uint4 buf[LS];                                   // all LS loads of the thread in flight before the first store
+#pragma unroll
+    for (int i = 0; i < LS; i++) {
+      const int idx = tid + i * 128, r = idx / LS, s = idx - r * LS;
+      const long st = site0 + r;
+      buf[i] = st < a.n_sites ? __ldg(a.in + st * (LS * 3) + s * 3 + c) : make_uint4(0, 0, 0, 0);
+    }
+#pragma unroll
+    for (int i = 0; i < LS; i++) {
+      const int idx = tid + i * 128, r = idx / LS, s = idx - r * LS;
+      *reinterpret_cast<uint4*>(As + (r >> 3) * Cfg::A_SBO + s * tc::A_LBO + (r & 7) * 16) = buf[i];
+    }
+    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+    asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+    const uint32_t tmem = tmem_slot;
+    if (tid == 0) {
+      const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(As), b0 = (uint32_t)__cvta_generic_to_shared(Bs);
+      constexpr uint32_t idesc = tc::idesc_f16(128, Cfg::N);
+#pragma unroll
+      for (int kk = 0; kk < Cfg::K / 16; kk++)
+        tc::mma_f16(tmem, tc::smem_desc(a0 + kk * 2 * tc::A_LBO, tc::A_LBO, Cfg::A_SBO), tc::smem_desc(b0 + kk * 256, 128, LS * 128), idesc, kk > 0);
+      tc::commit(bar);
+    }
+    mbar_wait(bar, (uint32_t)(c & 1));
+    asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+#pragma unroll
+    for (int s = 0; s < LS; s++) {
+      float v[8];
+      tc::ld8(tmem + ((uint32_t)(warp * 32) << 16) + s * 8, v);
+      uint4 q;
+      q.x = pack_h2(v[0], v[1]); q.y = pack_h2(v[2], v[3]); q.z = pack_h2(v[4], v[5]); q.w = pack_h2(v[6], v[7]);
+      if (site < a.n_sites) out4[s * 3 + c] = q;
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+    __syncthreads();                                 // A tile and accumulator are reused by the next colour
+  }
+  if (warp == 0) tc::tmem_free<DC::TMEM_COLS>(tmem_slot);
+}
+
 }  // namespace mspcg

@@ -310,3 +310,28 @@ def test_precond_fp16_more_blocks_than_resident_thread_blocks():
     r = synth.gaussian_spinor_abi(dims, Ls, 19)
     z = g.apply_precond(dev(torch, r), 3, F64).cpu().numpy()
     assert rel(z, ora.apply_precond(r, 3)) <= 2e-2
+
+
+# ---- the dense fifth-dimension contraction on its own: tcgen05 GEMM on an fp16 NATIVE vector ----
+@pytest.mark.parametrize("dims,Ls", [((4, 4, 4, 8), 8), ((6, 6, 6, 10), 12), ((8, 8, 6, 6), 16)])
+@pytest.mark.parametrize("dagger", [False, True])
+def test_M5inv_tcgen05_fp16(dims, Ls, dagger):
+    """mspcg_apply_M5inv against the oracle's M5^-1 (closed form R4) applied to the fp16-rounded input.
+    Site counts 256, 1080 and 1152: several 128-site tiles and a ragged tail.  Tolerance: the operands and the result are
+    rounded to fp16 (2^-11 each), accumulation is fp32 -> 2e-3 as for every fp16-storage operator."""
+    import torch
+    from oracle import mdwf
+    mf = 0.01
+    g = Mspcg(dims, Ls, MOB["b"], MOB["c"], MOB["M5"], mf, dims)
+    g.configure(F32, F16, 18)
+    v = synth.gaussian_spinor_abi(dims, Ls, 11)
+    nat = g.pack(dev(torch, v), F16)
+    v16 = g.unpack(nat, F16).cpu().numpy()                      # the rounded input, as the kernel sees it
+    out = g.unpack(g.apply_M5inv(nat, dagger), F16).cpu().numpy()
+    mob = mdwf.Mobius(Ls, MOB["b"], MOB["c"], MOB["M5"], mf)
+    ref = mdwf.pack_spinor_abi(mdwf.M5inv(mob, mdwf.unpack_spinor_abi(v16, dims, Ls), dagger), dims)
+    assert rel(out, ref) <= 2e-3
+    # M5^-1 M5 = 1 (north_star pin) seen from the GPU side: M5 of the oracle on the GPU result gives the input back
+    back = mdwf.pack_spinor_abi(mdwf.M5(mob, mdwf.unpack_spinor_abi(out, dims, Ls), dagger), dims)
+    assert rel(back, v16) <= 2e-3
+    g.close()
