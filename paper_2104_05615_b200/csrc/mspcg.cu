@@ -81,7 +81,7 @@ struct mspcg_ctx {
   double *rho = nullptr, *pq = nullptr; float* scale = nullptr; double* sc = nullptr;  // device scalars
   double* Tm = nullptr;          // device copy of the reduced-Ls transfer matrix T_host (A10)
   double* Gdev = nullptr;        // gradient accumulator of the T training (A12)
-  __half* Bm5[2] = {nullptr, nullptr};       // fp16 B-operand images of M5^-1 and M5^-dag for k_dense5d_tc
+  float* Bm5[2] = {nullptr, nullptr};        // chirality blocks of M5^-1 and M5^-dag (fp32 [hi][s][s']) for k_dense5d_tc
   __half *Bfwd = nullptr, *Bbwd = nullptr;   // fp16 B-operand images of T and T^dag for the tcgen05 transfer kernels
   bool transfer_tc = true;       // use them when (Ls, Ls_hat) is a compiled pair and the inner storage is fp16
   double* sc_host = nullptr;     // pinned
@@ -164,7 +164,7 @@ void carve(mspcg_ctx* c, Arena& a) {
   c->e_int_to_cb = a.take<int>(L.e_int_to_cb.size()); c->o_int_to_cb = a.take<int>(L.o_int_to_cb.size());
   c->negI = a.take<double>((size_t)2 * c->Ls * c->Ls);
   carve_mats(a, c->md, c->Ls); carve_mats(a, c->mf32, c->Ls); carve_frags(a, c->mfr);
-  for (int d = 0; d < 2; d++) c->Bm5[d] = a.take<__half>((size_t)64 * c->Ls * c->Ls);
+  for (int d = 0; d < 2; d++) c->Bm5[d] = a.take<float>((size_t)2 * c->Ls * c->Ls);
   if (c->Ls_hat) { carve_mats(a, c->md_hat, c->Ls_hat); carve_mats(a, c->mf32_hat, c->Ls_hat); carve_frags(a, c->mfr_hat); }
   c->rho = a.take<double>((size_t)(KMAX + 1) * L.nblk); c->pq = a.take<double>((size_t)KMAX * L.nblk);
   c->scale = a.take<float>(L.nblk); c->sc = a.take<double>(16);
@@ -541,20 +541,15 @@ template <typename V> cudaError_t up(void* dst, const std::vector<V>& src, cudaS
   return cudaMemcpyAsync(dst, src.data(), src.size() * sizeof(V), cudaMemcpyHostToDevice, st);
 }
 
-// fp16 B-operand images of M5^-1 (d = 0) and M5^-dag (d = 1) for k_dense5d_tc: B[n = (s, j)][k = (s', j')] = M_hi[s][s'] delta_jj',
-// j = (sp, hi, re/im), hi = (j >> 1) & 1; on P+ (hi = 0) M5^-1 is A+^-1 (hm.Ainv), on P- its transpose (R3); the dagger swaps them.
-// Same canonical K-major layout as the T images below.
+// The two chirality blocks of M5^-1 (d = 0) and M5^-dag (d = 1) for k_dense5d_tc, fp32 [hi][s][s']: on P+ (hi = 0) M5^-1 is A+^-1
+// (hm.Ainv), on P- its transpose (R3); the dagger swaps them.  The kernel rounds to fp16 and builds the MMA's B operand itself.
 int upload_m5_images(mspcg_ctx* ctx, cudaStream_t st) {
   const int Ls = ctx->Ls;
   for (int d = 0; d < 2; d++) {
-    std::vector<__half> img((size_t)64 * Ls * Ls, __float2half_rn(0.f));
-    for (int s = 0; s < Ls; s++) for (int sp = 0; sp < Ls; sp++) for (int j = 0; j < 8; j++) {
-      const int hi = (j >> 1) & 1;
-      const double v = ((hi ^ d) == 0) ? ctx->hm.Ainv.at(s, sp) : ctx->hm.Ainv.at(sp, s);
-      const int n = s * 8 + j, k = sp * 8 + j;
-      img[(size_t)(n / 8) * Ls * 64 + (size_t)(k / 8) * 64 + (n % 8) * 8 + (k % 8)] = __float2half_rn((float)v);
-    }
-    CUDA_OK(ctx, cudaMemcpyAsync(ctx->Bm5[d], img.data(), img.size() * sizeof(__half), cudaMemcpyHostToDevice, st));
+    std::vector<float> m((size_t)2 * Ls * Ls);
+    for (int hi = 0; hi < 2; hi++) for (int s = 0; s < Ls; s++) for (int sp = 0; sp < Ls; sp++)
+      m[((size_t)hi * Ls + s) * Ls + sp] = (float)(((hi ^ d) == 0) ? ctx->hm.Ainv.at(s, sp) : ctx->hm.Ainv.at(sp, s));
+    CUDA_OK(ctx, cudaMemcpyAsync(ctx->Bm5[d], m.data(), m.size() * sizeof(float), cudaMemcpyHostToDevice, st));
     CUDA_OK(ctx, cudaStreamSynchronize(st));
   }
   return MSPCG_OK;
@@ -1022,7 +1017,7 @@ int mspcg_apply_M5inv(mspcg_ctx* ctx, const void* in_dev, void* out_dev, int dag
   cudaStream_t st = (cudaStream_t)stream;
   Dense5dTcArgs a;
   a.in = reinterpret_cast<const uint4*>(in_dev); a.out = reinterpret_cast<uint4*>(out_dev);
-  a.Bimg = ctx->Bm5[dagger ? 1 : 0]; a.n_sites = (long)(v5h(ctx, ctx->Ls) / ctx->Ls);
+  a.M = ctx->Bm5[dagger ? 1 : 0]; a.n_sites = (long)(v5h(ctx, ctx->Ls) / ctx->Ls);
   const unsigned grid = (unsigned)((a.n_sites + tc::TILE - 1) / tc::TILE);
 #define DT(LSV)                                                                                                          \
   if (ctx->Ls == LSV) {                                                                                                  \

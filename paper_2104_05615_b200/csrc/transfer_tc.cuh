@@ -261,7 +261,7 @@ __global__ void __launch_bounds__(128, 1) k_reduce_end_tc(const TransferArgs a) 
 // north_star item 2): out[s][n] = sum_s' M_hi[s][s'] in[s'][n] on an fp16 NATIVE vector (layout of hop_mma.cuh:
 // v[site][s][colour][sp][hi][re,im]).  Per colour it is the GEMM  D[site][n] = sum_k A[site][k] B[n][k]  with
 // k = (s', j), n = (s, j), j = (sp, hi, re/im) the eight halves of one 16-byte chunk, and B[n][k] = M_hi[s][s'] delta_jj'
-// (host image, real).  The 16-byte chunk of one (site, s', colour) in HBM IS one core-matrix row of the K-major
+// (real, built in shared memory by the kernel).  The 16-byte chunk of one (site, s', colour) in HBM IS one core-matrix row of the K-major
 // canonical layout, so the A tile is filled with plain 128-bit copies, no conversion.  M = 128 sites per thread block,
 // N = K = 8 Ls, an N-column fp32 accumulator in tensor memory; the MMA does 8x the minimal flop count
 // (the delta_jj' zeros), which the tensor pipe does not notice at this size.
@@ -269,7 +269,7 @@ __global__ void __launch_bounds__(128, 1) k_reduce_end_tc(const TransferArgs a) 
 // serves the places where M5^-1 stands alone on an fp16 vector.
 struct Dense5dTcArgs {
   const uint4* in; uint4* out;   // NATIVE fp16 vectors, n_sites site columns of Ls*3 chunks
-  const __half* Bimg;            // B operand image [N/8][K/8][8][8]
+  const float* M;                // [hi][s][s'] the two chirality blocks of the matrix (fp32; rounded to fp16 in the kernel)
   long n_sites;
 };
 template <int LS> struct Dense5dTcCfg {
@@ -293,7 +293,15 @@ __global__ void __launch_bounds__(128, 3) k_dense5d_tc(const Dense5dTcArgs a) {
 
   if (warp == 0) tc::tmem_alloc<DC::TMEM_COLS>(&tmem_slot);
   if (tid == 0) { mbar_init(bar, 1); asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory"); }
-  for (int i = tid; i < Cfg::B_BYTES / 16; i += 128) reinterpret_cast<uint4*>(Bs)[i] = __ldg(reinterpret_cast<const uint4*>(a.Bimg) + i);
+  // B operand built in place from the two Ls x Ls chirality blocks (every thread block reading a 32 KB image from the same L2 lines
+  // was a hot spot): core matrix (s, s') = diag_j M_hi(j)[s][s'], row j is one 16-byte store with a single non-zero half.
+  for (int pr = tid; pr < LS * LS; pr += 128) {
+    const uint32_t m0 = (uint32_t)__half_as_ushort(__float2half_rn(__ldg(a.M + pr)));
+    const uint32_t m1 = (uint32_t)__half_as_ushort(__float2half_rn(__ldg(a.M + LS * LS + pr)));
+    uint4* d = reinterpret_cast<uint4*>(Bs) + pr * 8;
+    d[0] = make_uint4(m0, 0, 0, 0); d[1] = make_uint4(m0 << 16, 0, 0, 0); d[2] = make_uint4(0, m1, 0, 0); d[3] = make_uint4(0, m1 << 16, 0, 0);
+    d[4] = make_uint4(0, 0, m0, 0); d[5] = make_uint4(0, 0, m0 << 16, 0); d[6] = make_uint4(0, 0, 0, m1); d[7] = make_uint4(0, 0, 0, m1 << 16);
+  }
   const long site = site0 + tid;                     // epilogue: thread = TMEM lane = site row
   uint4* out4 = a.out + site * (LS * 3);
 #pragma unroll 1
