@@ -1018,7 +1018,8 @@ int mspcg_apply_M5inv(mspcg_ctx* ctx, const void* in_dev, void* out_dev, int dag
   Dense5dTcArgs a;
   a.in = reinterpret_cast<const uint4*>(in_dev); a.out = reinterpret_cast<uint4*>(out_dev);
   a.M = ctx->Bm5[dagger ? 1 : 0]; a.n_sites = (long)(v5h(ctx, ctx->Ls) / ctx->Ls);
-  const unsigned grid = (unsigned)((a.n_sites + tc::TILE - 1) / tc::TILE);
+  const long n_tiles = (a.n_sites + tc::TILE - 1) / tc::TILE;
+  const unsigned grid = (unsigned)(n_tiles < 2L * ctx->num_sms ? n_tiles : 2L * ctx->num_sms);   // persistent: two thread blocks per SM
 #define DT(LSV)                                                                                                          \
   if (ctx->Ls == LSV) {                                                                                                  \
     static bool attr = false;                                                                                            \

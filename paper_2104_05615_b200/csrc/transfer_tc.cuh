@@ -273,26 +273,28 @@ struct Dense5dTcArgs {
   long n_sites;
 };
 template <int LS> struct Dense5dTcCfg {
-  enum { N = 8 * LS, TMEM_COLS = (N <= 32 ? 32 : (N <= 64 ? 64 : (N <= 128 ? 128 : 256))),
-         SMEM = TransferCfg<LS, LS>::A_COLOUR + TransferCfg<LS, LS>::B_BYTES + 64 };
+  enum { N = 8 * LS, TMEM_COLS = (2 * N <= 32 ? 32 : (2 * N <= 64 ? 64 : (2 * N <= 128 ? 128 : (2 * N <= 256 ? 256 : 512)))),
+         SMEM = 2 * TransferCfg<LS, LS>::A_COLOUR + TransferCfg<LS, LS>::B_BYTES + 64 };
 };
-// One thread block = 128 sites; the three colours are processed one after the other through ONE A tile and ONE accumulator
-// (36 KB + 32 KB of shared memory and N of the 512 tensor-memory columns at Ls = 16), so that three thread blocks are resident
-// per SM and the load / MMA / write-back phases of different thread blocks overlap.
+// Persistent thread blocks (grid = min(tiles, 2 per SM)); a work item is (tile of 128 sites, colour).  Two A tiles and two
+// accumulators: the 16-byte chunks of item q+1 are fetched with cp.async (no registers, no wait) while the MMAs, the tensor-memory
+// read-back and the stores of item q run.  B is built once per thread block.
 template <int LS>
-__global__ void __launch_bounds__(128, 3) k_dense5d_tc(const Dense5dTcArgs a) {
+__global__ void __launch_bounds__(128, 2) k_dense5d_tc(const Dense5dTcArgs a) {
   typedef TransferCfg<LS, LS> Cfg;
   typedef Dense5dTcCfg<LS> DC;
   extern __shared__ __align__(128) unsigned char tsm[];
   __shared__ uint32_t tmem_slot;
-  unsigned char* As = tsm;
-  unsigned char* Bs = tsm + Cfg::A_COLOUR;
-  const uint32_t bar = (uint32_t)__cvta_generic_to_shared(tsm + Cfg::A_COLOUR + Cfg::B_BYTES);
+  unsigned char* Bs = tsm + 2 * Cfg::A_COLOUR;
+  const uint32_t as_u32 = (uint32_t)__cvta_generic_to_shared(tsm);
+  const uint32_t bar = (uint32_t)__cvta_generic_to_shared(tsm + 2 * Cfg::A_COLOUR + Cfg::B_BYTES);
   const int tid = threadIdx.x, warp = tid >> 5;
-  const long site0 = (long)blockIdx.x * tc::TILE;
+  const long n_tiles = (a.n_sites + tc::TILE - 1) / tc::TILE;
+  const long my_tiles = blockIdx.x < n_tiles ? (n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+  const long Q = 3 * my_tiles;
 
   if (warp == 0) tc::tmem_alloc<DC::TMEM_COLS>(&tmem_slot);
-  if (tid == 0) { mbar_init(bar, 1); asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory"); }
+  if (tid == 0) { mbar_init(bar, 1); mbar_init(bar + 8, 1); asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory"); }
   // B operand built in place from the two Ls x Ls chirality blocks (every thread block reading a 32 KB image from the same L2 lines
   // was a hot spot): core matrix (s, s') = diag_j M_hi(j)[s][s'], row j is one 16-byte store with a single non-zero half.
   for (int pr = tid; pr < LS * LS; pr += 128) {
@@ -302,48 +304,58 @@ __global__ void __launch_bounds__(128, 3) k_dense5d_tc(const Dense5dTcArgs a) {
     d[0] = make_uint4(m0, 0, 0, 0); d[1] = make_uint4(m0 << 16, 0, 0, 0); d[2] = make_uint4(0, m1, 0, 0); d[3] = make_uint4(0, m1 << 16, 0, 0);
     d[4] = make_uint4(0, 0, m0, 0); d[5] = make_uint4(0, 0, m0 << 16, 0); d[6] = make_uint4(0, 0, 0, m1); d[7] = make_uint4(0, 0, 0, m1 << 16);
   }
-  const long site = site0 + tid;                     // epilogue: thread = TMEM lane = site row
-  uint4* out4 = a.out + site * (LS * 3);
-#pragma unroll 1
-  for (int c = 0; c < 3; c++) {
-    uint4 buf[LS];                                   // all LS loads of the thread in flight before the first store
+  // asynchronous fetch of item q into A tile q & 1 (one commit group per item, empty past the end)
+  auto fetch = [&](long q) {
+    if (q < Q) {
+      const long site0 = ((long)blockIdx.x + (q / 3) * gridDim.x) * tc::TILE;
+      const int c = (int)(q % 3);
+      const uint32_t buf = as_u32 + (uint32_t)(q & 1) * Cfg::A_COLOUR;
 #pragma unroll
-    for (int i = 0; i < LS; i++) {
-      const int idx = tid + i * 128, r = idx / LS, s = idx - r * LS;
-      const long st = site0 + r;
-      buf[i] = st < a.n_sites ? __ldg(a.in + st * (LS * 3) + s * 3 + c) : make_uint4(0, 0, 0, 0);
+      for (int i = 0; i < LS; i++) {
+        const int idx = tid + i * 128, r = idx / LS, s = idx - r * LS;
+        const long st = site0 + r;
+        const uint32_t dst = buf + (r >> 3) * Cfg::A_SBO + s * tc::A_LBO + (r & 7) * 16;
+        if (st < a.n_sites) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(a.in + st * (LS * 3) + s * 3 + c) : "memory");
+        else asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};\n" ::"r"(dst), "r"(0u) : "memory");
+      }
     }
-#pragma unroll
-    for (int i = 0; i < LS; i++) {
-      const int idx = tid + i * 128, r = idx / LS, s = idx - r * LS;
-      *reinterpret_cast<uint4*>(As + (r >> 3) * Cfg::A_SBO + s * tc::A_LBO + (r & 7) * 16) = buf[i];
-    }
+    asm volatile("cp.async.commit_group;\n" ::: "memory");
+  };
+  fetch(0);
+  for (long q = 0; q < Q; q++) {
+    fetch(q + 1);                                    // its A tile was read by the MMAs of item q - 1, waited for below
+    asm volatile("cp.async.wait_group 1;\n" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
     asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-    const uint32_t tmem = tmem_slot;
+    const uint32_t tmem = tmem_slot + (uint32_t)(q & 1) * Cfg::N;
+    const uint32_t bq = bar + 8 * (uint32_t)(q & 1);
     if (tid == 0) {
-      const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(As), b0 = (uint32_t)__cvta_generic_to_shared(Bs);
+      const uint32_t a0 = as_u32 + (uint32_t)(q & 1) * Cfg::A_COLOUR, b0 = (uint32_t)__cvta_generic_to_shared(Bs);
       constexpr uint32_t idesc = tc::idesc_f16(128, Cfg::N);
 #pragma unroll
       for (int kk = 0; kk < Cfg::K / 16; kk++)
         tc::mma_f16(tmem, tc::smem_desc(a0 + kk * 2 * tc::A_LBO, tc::A_LBO, Cfg::A_SBO), tc::smem_desc(b0 + kk * 256, 128, LS * 128), idesc, kk > 0);
-      tc::commit(bar);
+      tc::commit(bq);
     }
-    mbar_wait(bar, (uint32_t)(c & 1));
+    mbar_wait(bq, (uint32_t)((q >> 1) & 1));
     asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+    const long site = ((long)blockIdx.x + (q / 3) * gridDim.x) * tc::TILE + tid;   // thread = TMEM lane = site row
+    const int c = (int)(q % 3);
+    uint4* out4 = a.out + site * (LS * 3);
 #pragma unroll
     for (int s = 0; s < LS; s++) {
       float v[8];
       tc::ld8(tmem + ((uint32_t)(warp * 32) << 16) + s * 8, v);
-      uint4 q;
-      q.x = pack_h2(v[0], v[1]); q.y = pack_h2(v[2], v[3]); q.z = pack_h2(v[4], v[5]); q.w = pack_h2(v[6], v[7]);
-      if (site < a.n_sites) out4[s * 3 + c] = q;
+      uint4 o;
+      o.x = pack_h2(v[0], v[1]); o.y = pack_h2(v[2], v[3]); o.z = pack_h2(v[4], v[5]); o.w = pack_h2(v[6], v[7]);
+      if (site < a.n_sites) out4[s * 3 + c] = o;
     }
-    asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-    __syncthreads();                                 // A tile and accumulator are reused by the next colour
   }
+  asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+  asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+  __syncthreads();
   if (warp == 0) tc::tmem_free<DC::TMEM_COLS>(tmem_slot);
 }
 
