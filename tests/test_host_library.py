@@ -93,3 +93,16 @@ def test_product_has_no_oracle_import():
             if f.endswith((".py", ".cu", ".cuh", ".hpp", ".h")):
                 txt = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in txt and "from oracle" not in txt and "liboracle" not in txt, f
+
+
+def test_apply_calls_fail_loudly_without_workspace(lib):
+    """Error behaviour stated in include/mspcg.h: compute entry points return an error code (never a CPU result) when
+    the workspace has not been set; checked through the raw C ABI with dummy non-null pointers (nothing is dereferenced)."""
+    import ctypes as C
+    m = Mspcg((4, 4, 4, 4), 8, 1.5, 0.5, 1.8, 0.01, (2, 2, 2, 2))
+    a, b = C.c_void_p(256), C.c_void_p(512)
+    assert lib.mspcg_apply_M5inv(m.h, a, b, 0, None) != 0
+    assert lib.mspcg_apply_MdagM(m.h, a, b, binding.F64, 0, None) != 0
+    assert lib.mspcg_apply_precond(m.h, a, b, binding.F64, 0, 6, 0, None) != 0
+    assert lib.mspcg_apply_M5inv(None, a, b, 0, None) != 0
+    m.close()
