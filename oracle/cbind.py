@@ -1,7 +1,7 @@
 """ctypes front end of Oracle-B (plain C, oracle/mdwf_oracle.c).  Test infrastructure only.
 
 Same ABI-level interface as oracle.Oracle (numpy Oracle-A); the two are independent
-restatements of the paper and are cross-checked in tests/test_oracle_cross.py.
+restatements of the paper and are cross-checked in tests/test_oracle_solvers.py (test_oracle_A_vs_B_cross_check).
 """
 from __future__ import annotations
 

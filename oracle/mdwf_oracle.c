@@ -472,7 +472,8 @@ int ora_solve(ora_t *o, const double *b_abi, double *x_abi, double tol, int max_
       }
       if (use_precond) precond_lat(o, r, z, n_inner, -1); else memcpy(z, r, n * sizeof(cplx));
       double rz2 = rdot(n, r, z);
-      double beta = replaced ? rz2 / rz : (rz2 + alpha * rdot(n, z, Ap)) / rz;
+      /* eq. 18: <z', r' - r>/<z, r> with r' - r = -alpha A p (the axpy above); Alg. 1's ratio right after a replacement (R16) */
+      double beta = replaced ? rz2 / rz : -alpha * rdot(n, z, Ap) / rz;
 #pragma omp parallel for schedule(static)
       for (long i = 0; i < (long)n; i++) p[i] = z[i] + beta * p[i];
       rz = rz2;

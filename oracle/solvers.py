@@ -7,7 +7,8 @@ code with the CUDA path.  Only tests/, __graft_entry__.smoke() and bench.py's cp
 Cites: Algorithm 1, eq. 12-14, fixed inner iteration
 count, Polak-Ribiere beta eq. 18, reliable updates (PAPER.md:283,
 rule = reading R17).  Pins: dense direct solves, "k >= dim block CG = A_s^-1", CG and MSPCG reach
-the same x (tests/test_oracle_solvers.py).
+the same x (tests/test_oracle_solvers.py); the outer loop's path (beta) by CG theory: finite termination,
+conjugacy, PR = FR for a fixed linear M, iteration counts of a textbook loop (tests/test_oracle_cg_theory.py).
 """
 from __future__ import annotations
 
@@ -163,9 +164,10 @@ def pcg(apply_A, b, precond=None, tol=1e-10, max_iter=100000, x0=None,
         z = precond(r_lo) if precond is not None else r_lo.copy()   # z_{k+1} = M^-1 r_{k+1}
         rz_new = rdot(r_lo, z)
         if replaced:
-            beta = rz_new / rz                # R16: plain ratio right after a replacement
+            beta = rz_new / rz                # R16: Alg. 1's ratio right after a replacement (r_k is no longer the predecessor)
         else:
-            beta = (rz_new + alpha * rdot(z, Ap)) / rz   # eq. 18 with r_{k+1}-r_k = -alpha_k A p_k (R16)
+            # eq. 18: <z_{k+1}, r_{k+1} - r_k>/<z_k, r_k>, and r_{k+1} - r_k = -alpha_k A p_k exactly (the line above)
+            beta = -alpha * rdot(z, Ap) / rz
         p = rnd(z + beta * p)                 # p_{k+1} = z_{k+1} + beta_k p_k
         rz = rz_new
     x = x_hi + x_lo
