@@ -774,7 +774,8 @@ int solve_impl(mspcg_ctx* c, const double* b_abi, double* x_abi, const mspcg_sol
       SOLVE_CUDA(dot2<TS>(c, z, rlo, Ap, nreal, st));
       SOLVE_CUDA(sc_read(c, 2, st));
       const double rz_new = c->sc_host[0], zAp = c->sc_host[1];
-      beta = replaced ? rz_new / rz : (rz_new + alpha * zAp) / rz;   // eq. 18 in the form of R16
+      // eq. 18: <z', r' - r>/<z, r> with r' - r = -alpha A p; Alg. 1's ratio right after a replacement (R16)
+      beta = replaced ? rz_new / rz : -alpha * zAp / rz;
       rz = rz_new;
     }
     if (!stt->converged && rc == MSPCG_OK) rc = MSPCG_ENOCONV;
