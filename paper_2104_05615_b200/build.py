@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmspcg.so")
 SOURCES = ["mspcg.cu"]
-DEPS = ["mspcg.cu", "kernels.cuh", "hop_mma.cuh", "transfer_tc.cuh", "site_math.cuh", "geometry.hpp", os.path.join("..", "..", "include", "mspcg.h")]
+DEPS = ["mspcg.cu", "kernels.cuh", "hop_mma.cuh", "hop_tile.cuh", "tile_tables.hpp", "transfer_tc.cuh", "site_math.cuh", "geometry.hpp", os.path.join("..", "..", "include", "mspcg.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

@@ -17,6 +17,7 @@
 // Direction code: dir = 2*mu + 0 -> neighbour x+mu (term (1 - g_mu) U_mu(x) psi(x+mu) of PAPER.md:105 eq. 8),
 //                 dir = 2*mu + 1 -> neighbour x-mu (term (1 + g_mu) U_mu(x-mu)^dag psi(x-mu)).
 #pragma once
+#include <algorithm>
 #include <cstdint>
 #include <cstdlib>
 #include <vector>
@@ -56,23 +57,36 @@ inline void build_block_geometry(Lattice& lat) {
     for (int d = 0; d < 4; d++) if (lat.cut[d]) { if (c[d] < 0) dsum += -c[d]; else if (c[d] >= lat.B[d]) dsum += c[d] - lat.B[d] + 1; }
     return dsum;
   };
-  // two passes per parity: interior (d = 0) first, then the halo, each in lexicographic order (x fastest)
-  for (int pass = 0; pass < 2; pass++) {
+  // List order: interior (d = 0) sites first, then the halo; inside each part sites are ordered by 4x4x2x2 CELL (cells in
+  // lexicographic order, x fastest) and lexicographically (x fastest) inside a cell, the same rule for both parities.  The
+  // sites of one cell and parity are therefore one contiguous run of the list, and so are the rows and planes of a cell that a
+  // neighbouring cell needs: the tile kernel (hop_tile.cuh, tile_tables.hpp) fetches a tile's inputs with few large copies.
+  {
+    const int cell[4] = {4, 4, 2, 2};
+    struct Ent { int pass; long key; long lex; int par; };
+    std::vector<Ent> ents;
+    ents.reserve(nbox);
     for (long i = 0; i < nbox; i++) {
       long r = i; int c[4];
       for (int d = 0; d < 4; d++) { c[d] = (int)(r % ext[d]) - off[d]; r /= ext[d]; }
-      int par = pmod(c[0] + c[1] + c[2] + c[3], 2);
-      int dd = overshoot(c);
-      if ((pass == 0) != (dd == 0)) continue;
-      if (par == 0 && dd <= 2) {
-        idx[i] = g.nE++;
-        for (int d = 0; d < 4; d++) g.cE.push_back((short)c[d]);
-      } else if (par == 1 && dd <= 1) {
-        idx[i] = g.nO++;
-        for (int d = 0; d < 4; d++) g.cO.push_back((short)c[d]);
-      }
+      const int par = pmod(c[0] + c[1] + c[2] + c[3], 2);
+      const int dd = overshoot(c);
+      if (!((par == 0 && dd <= 2) || (par == 1 && dd <= 1))) continue;
+      long key = 0;
+      for (int d = 3; d >= 0; d--) key = key * 4096 + (c[d] + 4) / cell[d];   // c >= -2, so c + 4 > 0 keeps cell 0 aligned at c = 0 (4 % cell == 0)
+      ents.push_back({dd == 0 ? 0 : 1, key, i, par});
     }
-    if (pass == 0) { g.nE0 = g.nE; g.nO0 = g.nO; }
+    std::sort(ents.begin(), ents.end(), [](const Ent& a, const Ent& b) {
+      if (a.pass != b.pass) return a.pass < b.pass;
+      if (a.key != b.key) return a.key < b.key;
+      return a.lex < b.lex;
+    });
+    for (const Ent& e : ents) {
+      long r = e.lex; int c[4];
+      for (int d = 0; d < 4; d++) { c[d] = (int)(r % ext[d]) - off[d]; r /= ext[d]; }
+      if (e.par == 0) { idx[e.lex] = g.nE++; for (int d = 0; d < 4; d++) g.cE.push_back((short)c[d]); if (e.pass == 0) g.nE0 = g.nE; }
+      else            { idx[e.lex] = g.nO++; for (int d = 0; d < 4; d++) g.cO.push_back((short)c[d]); if (e.pass == 0) g.nO0 = g.nO; }
+    }
   }
   auto neighbours = [&](const std::vector<short>& cs, int n, std::vector<int>& out) {
     out.assign((size_t)n * 8, -1);

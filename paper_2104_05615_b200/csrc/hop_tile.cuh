@@ -1,0 +1,293 @@
+// hop_tile.cuh -- the fused hop kernel for fp16 storage as a thread-block-cooperative TILE kernel (the preconditioner's
+// hot path; "the vector is loaded once into shared memory and reused by the stencil").
+//
+// k_hop_mma (hop_mma.cuh) gives every warp a private copy of the eight neighbour columns of its site: every input column
+// crosses L2 -> SM eight times, and at Ls = 16 (768 B per column) the kernel runs at the L2 slice throughput
+// (~12 TB/s) and not at the HBM roofline.  Here a persistent thread block owns a TILE of <= 32 output sites that are compact
+// in 4D (tile_tables.hpp) and stages the UNION of their neighbour columns once (<= 128 columns, 4.0 per output site on a
+// 4x4x2x2 cell instead of 8):
+//   * warps 0..NWP-1 are producers: for every tile they issue one TMA bulk copy (cp.async.bulk, SASS UBLKCP) per RUN of
+//     consecutive input columns (the lists are cell-ordered, geometry.hpp, so a 4x4x2x2 cell needs ~20 copies for its 128
+//     columns), one per run of output sites for their links, and one for the tile header, all completing on the stage's
+//     `full` mbarrier; two stages, so the copies of tile i+1 run while tile i is computed (a single warp issues a copy
+//     every ~45 cycles -- lane-serialised ELECT / R2UR / UBLKCP -- hence several producer warps);
+//   * the other NWC warps are consumers: warp w computes output sites w, w+NWC, ... of the tile with the arithmetic of
+//     hop_mma.cuh (half-spinor projection, SU(3) x half-spinor and the Ls x Ls matrices on the tensor cores with
+//     mma.m16n8k16, fp32 accumulation); neighbour fragments are 128-bit shared-memory reads at slot * column size;
+//     link words are 32-bit shared-memory reads; a consumer touches global memory only for the xpay / dot operands
+//     and for its stores.  When a warp is done with a stage it arrives on the stage's `empty` mbarrier.
+// Tiles are dealt to thread blocks in contiguous chunks of the flattened (Dirichlet block, tile) index, so a thread block
+// stays inside one Dirichlet block for many tiles (one atomic per warp and Dirichlet block for the fused <p, A p>).
+// Links carry the antiperiodic sign already (18 reals; the 12-real format keeps the per-warp kernel).
+#pragma once
+#include "tile_tables.hpp"
+
+namespace mspcg {
+
+template <int LS> struct TileCfg {
+  enum {
+    TS = TILE_TS, NIN = TILE_NIN, NWC = 16, NWP = 4, NSTAGE = 2,   // consumer warps, producer warps, pipeline stages
+    COL = LS * 48,                       // bytes of one site column
+    LINKREC = 8 * 18 * 2,                // bytes of the eight links of one output site
+    OFF_ZERO = NIN * COL,                // one column of zeros: the slot of every absent neighbour (and of the pad lanes' link words)
+    OFF_LINK = OFF_ZERO + COL,
+    OFF_HDR = OFF_LINK + TS * LINKREC,
+    STAGE = ((OFF_HDR + TILE_HDR + 127) / 128) * 128,
+    SMEM = NSTAGE * STAGE,
+    THREADS = 32 * (NWC + NWP),
+  };
+};
+
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];\n" : "=r"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ uint2 lds64(uint32_t addr) {
+  uint2 v;
+  asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];\n" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+  return v;
+}
+
+// Both half spinors of (1 + c gamma_mu) psi = (h, h'),  h = u + c G l,  h' = l + c G^dag u = c G^dag h  (G = -i sigma_k, 1 for
+// mu = t; c = -sg forward, +sg backward), are formed BEFORE the SU(3) product: upper += W h and lower += W h' are then two MMAs
+// with the same B fragment that accumulate over all eight directions, with no recombination arithmetic after the MMA
+// (hop_mma.cuh multiplies h only and maps W_b h_b - W_f h_f onto the lower components with 8 FMAs per direction pair and
+// segment).  chunk = {u0, l0, u1, l1}.
+template <int MU, bool FWD>
+__device__ __forceinline__ void project_lo(const uint4& q, const HsConst& k, uint32_t& h0, uint32_t& h1) {
+  if (MU == 0)      { const uint32_t m = FWD ? k.Q : k.R; h0 = hfma2_u32(swap_h2(q.z), m, q.y); h1 = hfma2_u32(swap_h2(q.x), m, q.w); }
+  else if (MU == 1) { h0 = hfma2_u32(q.z, FWD ? k.N : k.P, q.y); h1 = hfma2_u32(q.x, FWD ? k.P : k.N, q.w); }
+  else if (MU == 2) { h0 = hfma2_u32(swap_h2(q.x), FWD ? k.Q : k.R, q.y); h1 = hfma2_u32(swap_h2(q.z), FWD ? k.R : k.Q, q.w); }
+  else              { const uint32_t m = FWD ? k.N : k.P; h0 = hfma2_u32(q.x, m, q.y); h1 = hfma2_u32(q.z, m, q.w); }
+}
+template <int MU, int LS>
+__device__ __forceinline__ void hop_mu_full(float (&S)[MmaCfg<LS>::NMT][4], const uint4 (&F)[MmaCfg<LS>::NSEG], const uint4 (&B)[MmaCfg<LS>::NSEG],
+                                            uint32_t bf, uint32_t bb, const HsConst& k) {
+#pragma unroll
+  for (int seg = 0; seg < MmaCfg<LS>::NSEG; seg++) {
+    uint32_t f0, f1, b0, b1, g0, g1, c0, c1;
+    project_hs<MU, true>(F[seg], k, f0, f1);
+    project_hs<MU, false>(B[seg], k, b0, b1);
+    project_lo<MU, true>(F[seg], k, g0, g1);
+    project_lo<MU, false>(B[seg], k, c0, c1);
+    float (&S0)[4] = S[2 * seg], (&S1)[4] = S[2 * seg + 1];
+    mma16816_4(S0[0], S0[1], S1[0], S1[1], f0, f1, b0, b1, bf, bb);
+    mma16816_4(S0[2], S0[3], S1[2], S1[3], g0, g1, c0, c1, bf, bb);
+  }
+}
+
+template <int LS, int EPI>
+__global__ void __launch_bounds__(TileCfg<LS>::THREADS, 1) k_hop_tile(const HopArgs<__half> a) {
+  typedef MmaCfg<LS> Cfg;
+  typedef TileCfg<LS> TC;
+  constexpr int NSEG = Cfg::NSEG, NMT = Cfg::NMT, NWC = TC::NWC;
+  extern __shared__ __align__(128) unsigned char smraw[];
+  __shared__ uint4 sfrag[(EPI == EPI_K3 ? 2 : 1) * 64];   // A fragments of the 5D matrices
+  __shared__ __align__(8) uint64_t bars[2 * TC::NSTAGE];  // full[stage], empty[stage]
+  if (threadIdx.x < 64) sfrag[threadIdx.x] = __ldg(a.frag1 + threadIdx.x);
+  if (EPI == EPI_K3) { if (threadIdx.x >= 64 && threadIdx.x < 128) sfrag[threadIdx.x] = __ldg(a.frag2 + threadIdx.x - 64); }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t sm_u32 = smem_u32(smraw);
+  const uint32_t full_u32 = smem_u32(bars), empty_u32 = full_u32 + 8 * TC::NSTAGE;
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int s = 0; s < TC::NSTAGE; s++) { mbar_init(full_u32 + 8 * s, TC::NWP); mbar_init(empty_u32 + 8 * s, NWC); }
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+
+  const long total = (long)a.nblk * a.n_tiles;
+  const long per = (total + gridDim.x - 1) / gridDim.x;
+  const long t_begin = (long)blockIdx.x * per;
+  const long t_end = t_begin + per < total ? t_begin + per : total;
+
+  int blk0 = (int)(t_begin / a.n_tiles), ti0 = (int)(t_begin - (long)blk0 * a.n_tiles);
+  if (warp < TC::NWP) {
+    // ----------------------------------------------------------------------------------------------- producer warps
+    // Warp w fetches the input slots [w NIN/NWP, (w+1) NIN/NWP) (a lane issues a copy for each of its slots where a run starts)
+    // and the link records of the output sites [w TS/NWP, (w+1) TS/NWP); warp 0 also fetches the tile header.  Every producer warp posts
+    // the bytes of its own copies on the stage's `full` barrier (arrival count NWP) before it issues them.
+    int stage = 0, blk = blk0, ti = ti0;
+    uint32_t phases = 0xffffffffu;   // bit s: parity to wait for on empty[s]; a fresh barrier passes a wait on the phase before its first one
+    constexpr int SPW = TC::NIN / TC::NWP / 32;        // input slots per lane
+    constexpr int OPW = TC::TS / TC::NWP;              // output sites per producer warp
+    const int slot0 = (TC::NIN / TC::NWP) * warp + lane, oj = OPW * warp + (lane < OPW ? lane : 0);
+    for (long tt = t_begin; tt < t_end; tt++) {
+      const TileRec* rec = a.tiles + ti;
+      int col[SPW]; uint32_t run[SPW], nrun = 0;
+#pragma unroll
+      for (int q = 0; q < SPW; q++) { col[q] = __ldg(rec->in_col + slot0 + 32 * q); run[q] = __ldg(rec->in_run + slot0 + 32 * q); nrun += run[q]; }
+      const int osite = __ldg(rec->out_site + oj);
+      const uint32_t orun = lane < OPW ? (uint32_t)__ldg(rec->out_run + oj) : 0u;
+      const uint32_t sb = sm_u32 + stage * TC::STAGE, bar = full_u32 + 8 * stage;
+      const uint32_t bytes = __reduce_add_sync(0xffffffffu, nrun) * TC::COL + __reduce_add_sync(0xffffffffu, orun) * TC::LINKREC + (warp == 0 ? TILE_HDR : 0);
+      mbar_wait(empty_u32 + 8 * stage, (phases >> stage) & 1u);
+      if (lane == 0) {
+        mbar_expect_tx(bar, bytes);
+        if (warp == 0) bulk_g2s(sb + TC::OFF_HDR, rec, TILE_HDR, bar);
+      }
+      __syncwarp();
+      const unsigned char* inb = reinterpret_cast<const unsigned char*>(a.in) + (long)blk * a.in_stride * TC::COL;
+#pragma unroll
+      for (int q = 0; q < SPW; q++)
+        if (run[q]) bulk_g2s(sb + (slot0 + 32 * q) * TC::COL, inb + (long)col[q] * TC::COL, run[q] * TC::COL, bar);
+      if (orun)
+        bulk_g2s(sb + TC::OFF_LINK + oj * TC::LINKREC,
+                 reinterpret_cast<const unsigned char*>(a.links) + ((long)blk * a.link_stride + osite) * TC::LINKREC, orun * TC::LINKREC, bar);
+      phases ^= 1u << stage;
+      stage = stage + 1 == TC::NSTAGE ? 0 : stage + 1;
+      if (++ti == a.n_tiles) { ti = 0; blk++; }
+    }
+    return;
+  }
+
+  // -------------------------------------------------------------------------------------------------- consumer warps
+  const int cw = warp - TC::NWP;
+  const int g = lane >> 2, t = lane & 3;
+  HsConst hsk;
+  { const uint32_t p = a.sg > 0 ? 0x3c003c00u : 0xbc00bc00u, q = a.sg > 0 ? 0xbc003c00u : 0x3c00bc00u;   // half2 (sg, sg), (sg, -sg)
+    hsk.P = p; hsk.N = p ^ 0x80008000u; hsk.Q = q; hsk.R = q ^ 0x80008000u; }
+  // lane constants: fragment offset inside a site column (pad lanes clamped onto valid data, they meet zeros in B)
+  const int tt3 = t < 3 ? t : 2;
+  const int g0 = g < Cfg::N0 ? g : Cfg::N0 - 1;
+  const int g1 = Cfg::NSEG == 2 ? (g < Cfg::N1 ? g : Cfg::N1 - 1) : 0;
+  const int fo0 = g0 * 3 + tt3, fo1 = 24 + g1 * 3 + tt3;             // uint4 units
+  const bool st0 = t < 3 && g < Cfg::N0, st1 = Cfg::NSEG == 2 && t < 3 && g < Cfg::N1;
+  const bool lk_mine = t < 3 && g < 6;
+  const uint32_t lk_off = (uint32_t)(lk_mine ? ((g >> 1) * 3 + t) : 0);   // this lane's word inside an 18-real link
+  const uint32_t bsel = (g & 1) ? 0x1032u : 0x7610u;
+  const int lk_step = lk_mine ? 9 : 0;
+
+  float part = 0.f;
+  int part_blk = -1;
+  auto flush_dot = [&]() {
+    if (EPI == EPI_XPAY && a.dot_out != nullptr && part_blk >= 0) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+      if (lane == 0) atomicAdd(a.dot_out + (long)part_blk * a.dot_stride, (double)part);
+    }
+    part = 0.f;
+  };
+
+  int stage = 0;
+  uint32_t phases = 0u;              // bit s: parity to wait for on full[s]
+  {  // the zero column of both stages (never touched by the copies)
+    for (int s2 = 0; s2 < TC::NSTAGE; s2++) {
+      uint4* z = reinterpret_cast<uint4*>(smraw + s2 * TC::STAGE + TC::OFF_ZERO);
+      for (int i = threadIdx.x - 32 * TC::NWP; i < TC::COL / 16; i += 32 * NWC) z[i] = make_uint4(0, 0, 0, 0);
+    }
+    asm volatile("bar.sync 1, %0;\n" ::"n"(32 * NWC) : "memory");   // consumer warps only
+  }
+  int blk = blk0, ti = ti0;
+  for (long tt = t_begin; tt < t_end; tt++) {
+    if (blk != part_blk) { flush_dot(); part_blk = blk; }
+    const uint4* aux4 = nullptr; const uint4* dot4 = nullptr;
+    uint4* out4 = reinterpret_cast<uint4*>(a.out) + (long)blk * a.out_stride * (LS * 3);
+    uint4* out24 = nullptr;
+    if (EPI == EPI_K3) out24 = reinterpret_cast<uint4*>(a.out2) + (long)blk * a.out2_stride * (LS * 3);
+    if (EPI != EPI_PLAIN) aux4 = reinterpret_cast<const uint4*>(a.aux) + (long)blk * a.aux_stride * (LS * 3);
+    if (EPI == EPI_XPAY && a.dot_out) dot4 = reinterpret_cast<const uint4*>(a.dotv) + (long)blk * a.dotv_stride * (LS * 3);
+
+    const uint32_t sb = sm_u32 + stage * TC::STAGE;
+    mbar_wait(full_u32 + 8 * stage, (phases >> stage) & 1u);
+    const uint32_t hdr = sb + TC::OFF_HDR;
+    const uint4* stg4 = reinterpret_cast<const uint4*>(smraw + stage * TC::STAGE);
+    const uint32_t* lk32 = reinterpret_cast<const uint32_t*>(smraw + stage * TC::STAGE + TC::OFF_LINK);
+    const uint32_t* zero32 = reinterpret_cast<const uint32_t*>(smraw + stage * TC::STAGE + TC::OFF_ZERO);
+    const int n_out = (int)lds32(hdr);
+    for (int j = cw; j < n_out; j += NWC) {
+      const int site = (int)lds32(hdr + 16 + 4 * j);
+      const uint2 sl = lds64(hdr + 16 + 4 * TC::TS + 8 * j);
+      const unsigned have = (lds32(hdr + 16 + 12 * TC::TS + (j & ~3)) >> (8 * (j & 3))) & 0xffu;
+      uint4 dv[NSEG], av[NSEG];
+      if (EPI != EPI_PLAIN) {
+        const bool ok = site < a.n_aux;
+        const uint4* p = aux4 + (long)site * (LS * 3);
+        av[0] = (ok && st0) ? __ldg(p + fo0) : make_uint4(0, 0, 0, 0);
+        if (NSEG == 2) av[NSEG - 1] = (ok && st1) ? __ldg(p + fo1) : make_uint4(0, 0, 0, 0);
+      }
+      if (EPI == EPI_XPAY && dot4 != nullptr) {
+        const uint4* p = dot4 + (long)site * (LS * 3);
+        dv[0] = st0 ? __ldg(p + fo0) : make_uint4(0, 0, 0, 0);
+        if (NSEG == 2) dv[NSEG - 1] = st1 ? __ldg(p + fo1) : make_uint4(0, 0, 0, 0);
+      }
+      uint32_t bfr[8];
+      {  // B fragments: this lane's complex entry of each link as (Wr, -Wi) or (Wi, Wr); pad lanes read zeros
+        const uint32_t* lkb = lk_mine ? lk32 + j * (TC::LINKREC / 4) + lk_off : zero32;
+#pragma unroll
+        for (int d = 0; d < 8; d++) {
+          const uint32_t raw = lkb[d * lk_step];
+          bfr[d] = __byte_perm(raw, raw ^ 0x80000000u, bsel);
+        }
+      }
+      float S[NMT][4];
+#pragma unroll
+      for (int m = 0; m < NMT; m++) { S[m][0] = S[m][1] = S[m][2] = S[m][3] = 0.f; }
+#define MSPCG_TILE_MU(MU, COND)                                                                        \
+      if (COND) {                                                                                      \
+        uint4 Ff[NSEG], Bb[NSEG];                                                                      \
+        const uint32_t w2 = (MU < 2 ? sl.x : sl.y) >> (16 * (MU & 1));                                 \
+        const uint4* pf = stg4 + (w2 & 0xffu) * (TC::COL / 16);                                        \
+        const uint4* pb = stg4 + ((w2 >> 8) & 0xffu) * (TC::COL / 16);                                 \
+        Ff[0] = pf[fo0]; Bb[0] = pb[fo0];                                                              \
+        if (NSEG == 2) { Ff[NSEG - 1] = pf[fo1]; Bb[NSEG - 1] = pb[fo1]; }                             \
+        hop_mu_full<MU, LS>(S, Ff, Bb, bfr[2 * MU], bfr[2 * MU + 1], hsk);                           \
+      }
+      MSPCG_TILE_MU(0, have & 0x03u) MSPCG_TILE_MU(1, have & 0x0cu) MSPCG_TILE_MU(2, have & 0x30u) MSPCG_TILE_MU(3, have & 0xc0u)
+#undef MSPCG_TILE_MU
+
+      dense5d_mma<LS>(S, sfrag, lane);
+
+      uint4 o[NSEG];
+      uint4* po = out4 + (long)site * (LS * 3);
+      if (EPI == EPI_PLAIN) {
+        float_to_frag<LS>(S, o);
+        if (st0) po[fo0] = o[0];
+        if (NSEG == 2) { if (st1) po[fo1] = o[NSEG - 1]; }
+      } else {
+        float V[NMT][4];
+        frag_to_float<LS>(av, V);
+#pragma unroll
+        for (int m = 0; m < NMT; m++) {
+#pragma unroll
+          for (int q = 0; q < 4; q++) S[m][q] = V[m][q] - S[m][q];
+        }
+        float_to_frag<LS>(S, o);
+        if (EPI == EPI_K3) {
+          if (site < a.n_out2) {
+            uint4* p2 = out24 + (long)site * (LS * 3);
+            if (st0) p2[fo0] = o[0];
+            if (NSEG == 2) { if (st1) p2[fo1] = o[NSEG - 1]; }
+          }
+          dense5d_mma<LS>(S, sfrag + 64, lane);
+          float_to_frag<LS>(S, o);
+        }
+        if (st0) po[fo0] = o[0];
+        if (NSEG == 2) { if (st1) po[fo1] = o[NSEG - 1]; }
+        if (EPI == EPI_XPAY && dot4 != nullptr) {
+          float P[NMT][4];
+          frag_to_float<LS>(dv, P);
+          if (st0 || st1) {
+#pragma unroll
+            for (int m = 0; m < NMT; m++) {
+#pragma unroll
+              for (int q = 0; q < 4; q++) part += P[m][q] * S[m][q];
+            }
+          }
+        }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(empty_u32 + 8 * stage);
+    phases ^= 1u << stage;
+    stage = stage + 1 == TC::NSTAGE ? 0 : stage + 1;
+    if (++ti == a.n_tiles) { ti = 0; blk++; }
+  }
+  flush_dot();
+}
+
+}  // namespace mspcg

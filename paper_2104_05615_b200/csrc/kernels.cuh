@@ -15,6 +15,7 @@
 #include <stdint.h>
 
 #include "site_math.cuh"
+#include "tile_tables.hpp"
 
 namespace mspcg {
 
@@ -188,6 +189,7 @@ template <typename T> struct HopArgs {
   int nblk;                                        // fp16 path: Dirichlet blocks to walk (grid.y may be smaller)
   const C* mat1; const C* mat2;                    // device [2][LS][LS], transposed per chirality
   const uint4* frag1; const uint4* frag2;          // fp16 path: the same matrices as mma A fragments [2][32] (hop_mma.cuh)
+  const TileRec* tiles; int n_tiles;               // fp16 tile kernel (hop_tile.cuh): site tiles of this stage, shared by all blocks
   C sg;                                            // +1: D^w, -1: D^w^dag
 };
 
@@ -323,6 +325,7 @@ __global__ void __launch_bounds__(Tile<LS>::NT, (sizeof(typename ST<T>::C) == 8 
 
 }  // namespace mspcg
 #include "hop_mma.cuh"
+#include "hop_tile.cuh"
 namespace mspcg {
 
 // ------------------------------------------------------------------ K1: Mphi (bidiagonal in s), fused with p-updates
@@ -738,7 +741,8 @@ __device__ __forceinline__ void st_link_real(__half* p, double v) { *p = __float
 // Per-stage link copies: for list site i of block blk and dir = 2*mu+bw:
 //   bw = 0: W = U_mu(x);  bw = 1: W = U_mu(x - mu)^dag;  x = (origin(blk) + c_i) mod L, the GLOBAL periodic index
 // (reading R10: pad sites read links by global periodic index).  flip bit d set  <=>  the link crosses the
-// antiperiodic time boundary (R7).  Stored: first ng reals of W (ng = 12: two rows, R8).
+// antiperiodic time boundary (R7); with ng = 18 the sign is folded into the stored link instead and the bit stays clear.
+// Stored: first ng reals of W (ng = 12: two rows, R8).
 template <typename T>
 __global__ void k_build_links(const double* __restrict__ U_abi, T* __restrict__ links, uint8_t* __restrict__ flip,
                               const short* __restrict__ coords, const short* __restrict__ origin, long n_list, int nblk,
@@ -760,14 +764,16 @@ __global__ void k_build_links(const double* __restrict__ U_abi, T* __restrict__ 
       const int par = (y[0] + y[1] + y[2] + y[3]) & 1;
       const long lex = y[0] + (long)Lx * (y[1] + (long)Ly * (y[2] + (long)Lz * y[3]));
       const double* u = U_abi + (((long)mu * 2 + par) * Vh + lex / 2) * 18;
-      if (mu == 3 && tb == -1 && y[3] == Lt - 1) fl |= 1u << (2 * mu + bw);
+      // 18 stored reals: the sign is folded into the link; 12 reals: it must be applied after the third row is rebuilt (R7, R8)
+      double sgn = 1.0;
+      if (mu == 3 && tb == -1 && y[3] == Lt - 1) { if (ng == 18) sgn = -1.0; else fl |= 1u << (2 * mu + bw); }
       T* g = links + (idx * 8 + 2 * mu + bw) * ng;
       for (int q = 0; q < ng / 2; q++) {
         const int r = q / 3, c = q % 3;
         double re, im;
         if (!bw) { re = u[(r * 3 + c) * 2]; im = u[(r * 3 + c) * 2 + 1]; }
         else     { re = u[(c * 3 + r) * 2]; im = -u[(c * 3 + r) * 2 + 1]; }
-        st_link_real(g + 2 * q, re); st_link_real(g + 2 * q + 1, im);
+        st_link_real(g + 2 * q, sgn * re); st_link_real(g + 2 * q + 1, sgn * im);
       }
     }
   flip[idx] = (uint8_t)fl;

@@ -38,6 +38,13 @@ struct Arena {
 };
 
 struct GeomDev { int *nbrE = nullptr, *nbrO = nullptr; short *cE = nullptr, *cO = nullptr, *origin = nullptr; };
+// Site tiles of the fp16 tile kernel (hop_tile.cuh) for the four stage launches of one geometry: kernel 2 (O list, inputs
+// limited to the block interior), kernel 4 (O list), kernels 3 and 5 on the interior E sites, kernel 3 on the halo E sites.
+struct TileSet {
+  std::vector<TileRec> hO_lim, hO_all, hE_int, hE_halo;     // host
+  TileRec *O_lim = nullptr, *O_all = nullptr, *E_int = nullptr, *E_halo = nullptr;   // device
+  bool have = false;
+};
 
 // One set of fifth-dimension matrices (device, transposed per chirality: m[ch][s'][s]) in one compute type.
 template <typename C> struct MatSet { C *K2 = nullptr, *K3a = nullptr, *K3b = nullptr, *K4 = nullptr, *K5 = nullptr, *K3h = nullptr; };
@@ -73,6 +80,8 @@ struct mspcg_ctx {
   size_t ws_bytes = 0;
   // device
   GeomDev gfull, gblk;
+  TileSet tfull, tblk;
+  bool use_tiles = true;         // MSPCG_TILE=0 in the environment selects the per-warp kernel k_hop_mma (A/B measurements)
   int *e_int_to_cb = nullptr, *o_int_to_cb = nullptr;   // FULL list index -> ABI x_cb, even / odd parity
   double* negI = nullptr;        // device [2][Ls][Ls]: minus the identity (full 2x2 operator of eq. 4, mspcg_apply_full)
   MatSet<double> md, md_hat; MatSet<float> mf32, mf32_hat; MatFrag mfr, mfr_hat;
@@ -158,9 +167,23 @@ void carve_temps(Arena& a, OpBuf& o, const Geometry& g, int Ls) {   // stage vec
 //     the sloppy operator, of the block operator and the inner-CG vectors (none holds data between two calls);
 //   * the staging buffers of the ABI-layout and *_host entry points overlay the solver's fp64 vectors (a solve and an apply
 //     call never run at the same time on one context).
+void carve_tiles(Arena& a, TileSet& t) {
+  if (!t.have) return;
+  t.O_lim = a.take<TileRec>(t.hO_lim.size()); t.O_all = a.take<TileRec>(t.hO_all.size());
+  t.E_int = a.take<TileRec>(t.hE_int.size()); t.E_halo = a.take<TileRec>(t.hE_halo.size());
+}
+void build_tile_set(TileSet& t, const Geometry& g) {
+  if (t.have) return;
+  t.hO_lim = build_tiles(g.cO, g.nbrO, 0, g.nO, g.nE0);
+  if (g.nE0 == g.nE) t.hO_all.clear(); else t.hO_all = build_tiles(g.cO, g.nbrO, 0, g.nO, g.nE);   // FULL: kernel 4 uses kernel 2's tiles
+  t.hE_int = build_tiles(g.cE, g.nbrE, 0, g.nE0, g.nO);
+  t.hE_halo = build_tiles(g.cE, g.nbrE, g.nE0, g.nE, g.nO);
+  t.have = true;
+}
 void carve(mspcg_ctx* c, Arena& a) {
   const Lattice& L = c->lat;
   carve_geom(a, c->gfull, L.full); carve_geom(a, c->gblk, L.blk);
+  carve_tiles(a, c->tfull); carve_tiles(a, c->tblk);
   c->e_int_to_cb = a.take<int>(L.e_int_to_cb.size()); c->o_int_to_cb = a.take<int>(L.o_int_to_cb.size());
   c->negI = a.take<double>((size_t)2 * c->Ls * c->Ls);
   carve_mats(a, c->md, c->Ls); carve_mats(a, c->mf32, c->Ls); carve_frags(a, c->mfr);
@@ -222,7 +245,19 @@ cudaError_t launch_hop(mspcg_ctx* c, const HopArgs<T>& a, int nblk, cudaStream_t
   const bool was_timing = c->timing;
   if (!timed) c->timing = false;   // the caller times a group of launches as one (kernel 3 = interior + halo launch)
   const int kind = EPI == EPI_PLAIN ? KIND_HOP_PLAIN : (EPI == EPI_K3 ? KIND_HOP_K3 : KIND_HOP_XPAY);
-  if constexpr (std::is_same<T, __half>::value) {   // fp16 storage: warp-per-site tensor-core kernel (hop_mma.cuh)
+  if constexpr (std::is_same<T, __half>::value) {   // fp16 storage: tensor-core kernels (hop_tile.cuh, hop_mma.cuh)
+    if (a.tiles != nullptr && a.n_tiles > 0 && a.ng == 18) {   // thread-block-cooperative tile kernel
+      static bool tattr = false;
+      const size_t tsm = TileCfg<LS>::SMEM;
+      if (!tattr) { cudaFuncSetAttribute(k_hop_tile<LS, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsm); tattr = true; }
+      HopArgs<__half> ab = a; ab.nblk = nblk;
+      const long total = (long)nblk * a.n_tiles;
+      const unsigned grid = (unsigned)(total < c->num_sms ? total : c->num_sms);   // persistent: one thread block per SM
+      { TimedLaunch tl(c, kind, st); k_hop_tile<LS, EPI><<<grid, TileCfg<LS>::THREADS, tsm, st>>>(ab); }
+      c->launches++;
+      c->timing = was_timing;
+      return cudaPeekAtLastError();
+    }
     constexpr int NW = MmaCfg<LS>::NW;
     static bool attr = false;
     const size_t sm = MmaSmem<LS>::BLOCK;
@@ -274,9 +309,18 @@ template <typename T> struct OpView {
   const int *nbrE, *nbrO;
   const T *linksE, *linksO; const uint8_t *flipE, *flipO;
   T *t1, *tO, *y, *w;
+  const TileRec *tO_lim = nullptr, *tO_all = nullptr, *tE_int = nullptr, *tE_halo = nullptr;   // fp16 tile kernel
+  int ntO_lim = 0, ntO_all = 0, ntE_int = 0, ntE_halo = 0;
 };
 template <typename T> OpView<T> make_view(const mspcg_ctx* c, const OpBuf& o, const Geometry& g, const GeomDev& gd, int Ls, bool hat) {
   OpView<T> v;
+  const TileSet& ts = (&g == &c->lat.full) ? c->tfull : c->tblk;
+  if (sizeof(T) == 2 && ts.have && c->use_tiles && o.ng == 18) {
+    v.tO_lim = ts.O_lim; v.ntO_lim = (int)ts.hO_lim.size();
+    v.tO_all = ts.hO_all.empty() ? ts.O_lim : ts.O_all; v.ntO_all = ts.hO_all.empty() ? (int)ts.hO_lim.size() : (int)ts.hO_all.size();
+    v.tE_int = ts.E_int; v.ntE_int = (int)ts.hE_int.size();
+    v.tE_halo = ts.E_halo; v.ntE_halo = (int)ts.hE_halo.size();
+  }
   v.nblk = g.nblk; v.nE0 = g.nE0; v.nE = g.nE; v.nO = g.nO; v.ng = o.ng; v.Ls = Ls; v.hat = hat;
   v.nbrE = gd.nbrE; v.nbrO = gd.nbrO;
   v.linksE = (const T*)o.linksE; v.linksO = (const T*)o.linksO; v.flipE = o.flipE; v.flipO = o.flipO;
@@ -311,6 +355,7 @@ cudaError_t apply_normal(mspcg_ctx* c, const OpView<T>& v, MphiArgs<T> mp, const
   // K2
   a.in = v.t1; a.in_stride = v.nE0; a.n_in_limit = v.nE0; a.out = v.tO; a.out_stride = v.nO; a.n_out = v.nO;
   a.nbr = v.nbrO; a.links = v.linksO; a.flip = v.flipO; a.link_stride = v.nO; a.mat1 = m.K2; a.frag1 = mf.K2; a.sg = (C)1;
+  a.tiles = v.tO_lim; a.n_tiles = v.ntO_lim;
   if ((e = launch_hop<T, LS, EPI_PLAIN>(c, a, v.nblk, st)) != cudaSuccess) return e;
   // K3: on the interior sites (d = 0) y = p - M5^-1 D^w tO, w = M5^-dag y; on the halo sites of a Dirichlet block p = 0 and y is
   // not needed, so w = -(M5^-dag M5^-1) D^w tO is one contraction with the product matrix (a plain-epilogue launch on the site
@@ -318,6 +363,7 @@ cudaError_t apply_normal(mspcg_ctx* c, const OpView<T>& v, MphiArgs<T> mp, const
   a.in = v.tO; a.in_stride = v.nO; a.n_in_limit = v.nO; a.out = v.w; a.out_stride = v.nE; a.n_out = v.nE0;
   a.out2 = v.y; a.out2_stride = v.nE0; a.n_out2 = v.nE0; a.aux = p; a.aux_stride = v.nE0; a.n_aux = v.nE0;
   a.nbr = v.nbrE; a.links = v.linksE; a.flip = v.flipE; a.link_stride = v.nE; a.mat1 = m.K3a; a.mat2 = m.K3b; a.frag1 = mf.K3a; a.frag2 = mf.K3b;
+  a.tiles = v.tE_int; a.n_tiles = v.ntE_int;
   {
     TimedLaunch tl(c, KIND_HOP_K3, st);
     if ((e = launch_hop<T, LS, EPI_K3>(c, a, v.nblk, st, false)) != cudaSuccess) return e;
@@ -327,6 +373,8 @@ cudaError_t apply_normal(mspcg_ctx* c, const OpView<T>& v, MphiArgs<T> mp, const
       h.out2 = nullptr; h.n_out2 = 0; h.aux = nullptr; h.n_aux = 0;
       h.nbr = v.nbrE + (size_t)v.nE0 * 8; h.links = v.linksE + (size_t)v.nE0 * 8 * v.ng; h.flip = v.flipE + v.nE0;
       h.mat1 = m.K3h; h.mat2 = nullptr; h.frag1 = mf.K3h; h.frag2 = nullptr;
+      h.tiles = v.tE_halo; h.n_tiles = v.ntE_halo;
+      if (h.tiles != nullptr && h.n_tiles > 0) { h.out = v.w; h.links = v.linksE; }   // the tile tables carry absolute list indices
       if ((e = launch_hop<T, LS, EPI_PLAIN>(c, h, v.nblk, st, false)) != cudaSuccess) return e;
     }
   }
@@ -334,11 +382,13 @@ cudaError_t apply_normal(mspcg_ctx* c, const OpView<T>& v, MphiArgs<T> mp, const
   a.in = v.w; a.in_stride = v.nE; a.n_in_limit = v.nE; a.out = v.tO; a.out_stride = v.nO; a.n_out = v.nO;
   a.out2 = nullptr; a.aux = nullptr; a.n_aux = 0; a.nbr = v.nbrO; a.links = v.linksO; a.flip = v.flipO; a.link_stride = v.nO;
   a.mat1 = m.K4; a.mat2 = nullptr; a.frag1 = mf.K4; a.frag2 = nullptr; a.sg = (C)-1;
+  a.tiles = v.tO_all; a.n_tiles = v.ntO_all;
   if ((e = launch_hop<T, LS, EPI_PLAIN>(c, a, v.nblk, st)) != cudaSuccess) return e;
   // K5
   a.in = v.tO; a.in_stride = v.nO; a.n_in_limit = v.nO; a.out = q; a.out_stride = v.nE0; a.n_out = v.nE0;
   a.aux = v.y; a.aux_stride = v.nE0; a.n_aux = v.nE0; a.dotv = p; a.dotv_stride = v.nE0; a.dot_out = dot_out; a.dot_stride = 1;
   a.nbr = v.nbrE; a.links = v.linksE; a.flip = v.flipE; a.link_stride = v.nE; a.mat1 = m.K5; a.frag1 = mf.K5;
+  a.tiles = v.tE_int; a.n_tiles = v.ntE_int;
   return launch_hop<T, LS, EPI_XPAY>(c, a, v.nblk, st);
 }
 
@@ -900,7 +950,8 @@ int mspcg_create(mspcg_ctx** out, int Lx, int Ly, int Lz, int Lt, int Ls, double
   const int L[4] = {Lx, Ly, Lz, Lt}, B[4] = {Bx, By, Bz, Bt};
   if (!build_lattice(ctx->lat, L, B)) { delete ctx; return MSPCG_EINVAL; }
   ctx->Ls = Ls; ctx->b = b; ctx->c = c; ctx->M5 = M5; ctx->mf = mf;
-  { const char* e = getenv("MSPCG_TRANSFER_TC"); if (e && e[0] == '0') ctx->transfer_tc = false; }   // debugging switch: generic transfer kernels
+  { const char* e = getenv("MSPCG_TRANSFER_TC"); if (e && e[0] == '0') ctx->transfer_tc = false; }
+  { const char* e = getenv("MSPCG_TILE"); if (e && e[0] == '0') ctx->use_tiles = false; }             // A/B switch: per-warp hop kernel   // debugging switch: generic transfer kernels
   ctx->alpha = b * (4.0 - M5) + 1.0; ctx->beta = c * (4.0 - M5) - 1.0;
   if (!build_host_mats(ctx->hm, Ls, b, c, M5, mf)) { delete ctx; return MSPCG_EINVAL; }
   *out = ctx;
@@ -945,6 +996,10 @@ int mspcg_workspace_bytes(mspcg_ctx* ctx, int outer_prec, int inner_prec, int re
   if (!prec_ok(outer_prec) || !prec_ok(inner_prec) || (recon != 18 && recon != 12)) return fail(ctx, MSPCG_EINVAL, "bad precision or recon");
   if (ctx->have_ws) return fail(ctx, MSPCG_EINVAL, "workspace already set");
   ctx->outer_prec = outer_prec; ctx->inner_prec = inner_prec; ctx->recon = recon; ctx->configured = true;
+  if (ctx->use_tiles && recon == 18) {   // site tiles of the fp16 tile kernel, for the geometries that run in fp16
+    if (inner_prec == MSPCG_F16) build_tile_set(ctx->tblk, ctx->lat.blk);
+    if (outer_prec == MSPCG_F16) build_tile_set(ctx->tfull, ctx->lat.full);
+  }
   Arena a;
   carve(ctx, a);
   ctx->ws_bytes = (a.off + 255) & ~(size_t)255;
@@ -967,6 +1022,13 @@ int mspcg_set_workspace(mspcg_ctx* ctx, void* workspace_dev, size_t bytes, void*
   CUDA_OK(ctx, up(ctx->gblk.cE, L.blk.cE, st)); CUDA_OK(ctx, up(ctx->gblk.cO, L.blk.cO, st));
   CUDA_OK(ctx, up(ctx->gblk.origin, L.blk.origin, st));
   CUDA_OK(ctx, up(ctx->e_int_to_cb, L.e_int_to_cb, st)); CUDA_OK(ctx, up(ctx->o_int_to_cb, L.o_int_to_cb, st));
+  for (TileSet* t : {&ctx->tfull, &ctx->tblk}) {
+    if (!t->have) continue;
+    if (!t->hO_lim.empty()) CUDA_OK(ctx, up(t->O_lim, t->hO_lim, st));
+    if (!t->hO_all.empty()) CUDA_OK(ctx, up(t->O_all, t->hO_all, st));
+    if (!t->hE_int.empty()) CUDA_OK(ctx, up(t->E_int, t->hE_int, st));
+    if (!t->hE_halo.empty()) CUDA_OK(ctx, up(t->E_halo, t->hE_halo, st));
+  }
   { std::vector<double> ni((size_t)2 * ctx->Ls * ctx->Ls, 0.0);
     for (int ch = 0; ch < 2; ch++) for (int i = 0; i < ctx->Ls; i++) ni[((size_t)ch * ctx->Ls + i) * ctx->Ls + i] = -1.0;
     CUDA_OK(ctx, up(ctx->negI, ni, st)); }
