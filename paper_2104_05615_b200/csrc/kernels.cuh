@@ -337,7 +337,7 @@ template <typename T> struct MphiArgs {
   const T* in; T* p; T* t;          // mode 0: in -> t;  mode 1/2: in = z or r, p updated in place, t = Mphi p
   long n_sites;                     // sites per block (stride of all three arrays)
   int mode, it, nblk;
-  double beta;
+  double beta; const double* beta_dev;   // mode 1: beta by value, or read from device memory when beta_dev != null
   const double* rho; const double* pq;   // inner-CG scalars [it][nblk]
   C diag, off, mf;                  // Mphi = diag*1 + off*(P+ S_minus + P- S_plus), wrap factor -mf
 };
@@ -367,7 +367,7 @@ __global__ void __launch_bounds__(Tile<LS>::NT) k_mphi(const MphiArgs<T> a) {
   if (a.mode != 0) {
     C beta = 0;
     bool have_p = true;
-    if (a.mode == 1) beta = (C)a.beta;
+    if (a.mode == 1) beta = a.beta_dev ? (C)*a.beta_dev : (C)a.beta;
     else if (a.it == 0) have_p = false;
     else {
       const bool ok = inner_alive(a.rho, a.pq, a.nblk, blk, a.it - 1);
@@ -653,18 +653,22 @@ template <typename T> __device__ __forceinline__ void stchunk(T* base, long i, c
   typedef typename ST<T>::V V; V q; packV(q, v); reinterpret_cast<V*>(base)[i] = q;
 }
 
-// Outer-iteration BLAS-1 (Algorithm 1): alpha = <r,z> / <p,Ap> with <p,Ap> read from device memory (no host
-// round trip between the operator and this kernel; alpha = 0 if <p,Ap> <= 0, the host reports the breakdown),
-// x += alpha p, r -= alpha Ap, out[0] += |r|^2.
+// Device-resident scalars of the outer iteration (Algorithm 1; eq. 18): no host round trip between the kernels.
+//   sc[0] <p,Ap> (kernel 5)   sc[1] |r_{k+1}|^2   sc[2] <z_{k+1},r_{k+1}>   sc[3] <z_{k+1},A p_k>   (accumulators, zeroed by k_outer_scalars)
+//   sc[4] <z_k,r_k>   sc[5] alpha_k   sc[6] beta_k   sc[7] <z,r> before the last k_outer_scalars (denominator for a redo after a replacement)
+enum { SC_PAP = 0, SC_RR = 1, SC_RZN = 2, SC_ZAP = 3, SC_RZ = 4, SC_ALPHA = 5, SC_BETA = 6, SC_RZ_PREV = 7, SC_N = 8 };
+
+// alpha = <r,z> / <p,Ap> (0 if <p,Ap> <= 0: the host reports the breakdown), x += alpha p, r -= alpha Ap, sc[SC_RR] += |r|^2.
+// self_z (plain CG, z = r): also sc[SC_RZN] += |r|^2 and sc[SC_ZAP] += <r, Ap>, the two inner products of eq. 18, in the same pass.
 template <typename T>
 __global__ void k_outer_update(const T* __restrict__ p, const T* __restrict__ q, T* __restrict__ r, T* __restrict__ x,
-                               long nchunk, double rz, const double* __restrict__ pAp, double* out) {
+                               long nchunk, double* __restrict__ sc, int self_z) {
   __shared__ double red[32];
   constexpr int PER = ST<T>::PER;
-  const double pq = *pAp;
-  const double alpha = pq > 0.0 ? rz / pq : 0.0;
+  const double pq = sc[SC_PAP];
+  const double alpha = pq > 0.0 ? sc[SC_RZ] / pq : 0.0;
   const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
-  double part = 0;
+  double part = 0, part2 = 0;
   if (i < nchunk) {
     typename ST<T>::C vp[PER], vq[PER], vr[PER], vx[PER];
     ldchunk<T>(p, i, vp); ldchunk<T>(q, i, vq); ldchunk<T>(r, i, vr); ldchunk<T>(x, i, vx);
@@ -673,11 +677,40 @@ __global__ void k_outer_update(const T* __restrict__ p, const T* __restrict__ q,
       vx[k] = (typename ST<T>::C)((double)vx[k] + alpha * (double)vp[k]);
       vr[k] = round_store((typename ST<T>::C)((double)vr[k] - alpha * (double)vq[k]), (int)sizeof(T));
       part += (double)vr[k] * (double)vr[k];
+      part2 += (double)vr[k] * (double)vq[k];
     }
     stchunk<T>(x, i, vx); stchunk<T>(r, i, vr);
   }
   const double tot = block_sum(part, red, threadIdx.x, blockDim.x);
-  if (threadIdx.x == 0) atomicAdd(out, tot);
+  __syncthreads();
+  const double tot2 = self_z ? block_sum(part2, red, threadIdx.x, blockDim.x) : 0.0;
+  if (threadIdx.x == 0) {
+    atomicAdd(sc + SC_RR, tot);
+    if (self_z) { atomicAdd(sc + SC_RZN, tot); atomicAdd(sc + SC_ZAP, tot2); }
+    if (blockIdx.x == 0) sc[SC_ALPHA] = alpha;
+  }
+}
+
+// End of an outer iteration, one thread: beta_k of eq. 18, <z,r> <- <z',r'>, snapshot of (<p,Ap>, |r|^2) for the
+// host's lagged polling, accumulators cleared for the next iteration.
+//   mode 0: beta = -alpha <z',Ap> / <z,r>     (eq. 18 with r' - r = -alpha A p)
+//   mode 1: beta = <z',r'> / (f2 * <z,r>)     right after a residual replacement (Alg. 1's ratio, R16); f2 = (sigma_old/sigma_new)^2
+//           rescales <z,r> to the new unit of the fp16 sloppy vectors (R17b), 1 otherwise
+//   mode 2: as mode 1 but against the <z,r> saved before the previous call (the z of the replaced residual is recomputed)
+//   mode 3: start: <z,r> <- <z_0,r_0>, beta = 0
+__global__ void k_outer_scalars(double* __restrict__ sc, double* __restrict__ snap, int mode, double f2) {
+  const double rzn = sc[SC_RZN];
+  if (snap) { snap[0] = sc[SC_PAP]; snap[1] = sc[SC_RR]; }
+  if (mode == 3) { sc[SC_RZ] = rzn; sc[SC_RZ_PREV] = rzn; sc[SC_BETA] = 0.0; }
+  else {
+    const double rz = mode == 2 ? sc[SC_RZ_PREV] : sc[SC_RZ];
+    double beta;
+    if (mode == 0) beta = -sc[SC_ALPHA] * sc[SC_ZAP] / rz; else beta = rzn / (f2 * rz);
+    if (!(rz != 0.0)) beta = 0.0;
+    if (mode != 2) sc[SC_RZ_PREV] = rz;
+    sc[SC_BETA] = beta; sc[SC_RZ] = rzn;
+  }
+  sc[SC_PAP] = 0.0; sc[SC_RR] = 0.0; sc[SC_RZN] = 0.0; sc[SC_ZAP] = 0.0;
 }
 
 // out[0] += <a,b>, out[1] += <a,c> (c may be null): the inner products of the Polak-Ribiere beta (eq. 18, R16).

@@ -640,10 +640,10 @@ cudaError_t sc_read(mspcg_ctx* c, int n, cudaStream_t st) {
   if (e != cudaSuccess) return e;
   return cudaStreamSynchronize(st);
 }
-template <typename T> cudaError_t dot2(mspcg_ctx* c, const T* a, const T* b, const T* cc, long nreal, cudaStream_t st) {
+template <typename T> cudaError_t dot2(mspcg_ctx* c, const T* a, const T* b, const T* cc, long nreal, cudaStream_t st, double* out = nullptr) {
   const long nchunk = nreal / ST<T>::PER;
   long blocks = (nchunk + 255) / 256; if (blocks > 148 * 16) blocks = 148 * 16;
-  k_dot2<T><<<(unsigned)blocks, 256, 0, st>>>(a, b, cc, nchunk, c->sc);
+  k_dot2<T><<<(unsigned)blocks, 256, 0, st>>>(a, b, cc, nchunk, out ? out : c->sc);
   c->launches++;
   return cudaPeekAtLastError();
 }
@@ -744,10 +744,10 @@ int solve_impl(mspcg_ctx* c, const double* b_abi, double* x_abi, const mspcg_sol
   SOLVE_CUDA(cudaEventRecord(ev0, st));
   SOLVE_CUDA(pack_any(c, b_abi, b, MSPCG_F64, 1, st));
   SOLVE_CUDA(pack_any(c, x_abi, xhi, MSPCG_F64, 1, st));
-  SOLVE_CUDA(sc_zero(c, 2, st));
-  SOLVE_CUDA(dot2<double>(c, b, b, nullptr, nreal, st));
-  SOLVE_CUDA(sc_read(c, 1, st));
-  const double bnorm = std::sqrt(c->sc_host[0]);
+  SOLVE_CUDA(sc_zero(c, 16, st));
+  SOLVE_CUDA(dot2<double>(c, b, b, nullptr, nreal, st, c->sc + 8));
+  SOLVE_CUDA(sc_read(c, 16, st));
+  const double bnorm = std::sqrt(c->sc_host[8]);
   int k = 0, rc = MSPCG_OK;
   auto true_residual = [&](double* rn) -> cudaError_t {   // rhi = b - A xhi in fp64; *rn = |rhi|
     cudaError_t e;
@@ -755,17 +755,17 @@ int solve_impl(mspcg_ctx* c, const double* b_abi, double* x_abi, const mspcg_sol
     stt->outer_applies++;
     if ((e = cudaMemcpyAsync(rhi, b, sizeof(double) * nreal, cudaMemcpyDeviceToDevice, st)) != cudaSuccess) return e;
     if ((e = axpby<double>(c, -1.0, t64, 1.0, rhi, nreal, st)) != cudaSuccess) return e;
-    if ((e = sc_zero(c, 1, st)) != cudaSuccess) return e;
-    if ((e = dot2<double>(c, rhi, rhi, nullptr, nreal, st)) != cudaSuccess) return e;
-    if ((e = sc_read(c, 1, st)) != cudaSuccess) return e;
-    *rn = std::sqrt(c->sc_host[0]);
+    if ((e = cudaMemsetAsync(c->sc + 8, 0, sizeof(double), st)) != cudaSuccess) return e;
+    if ((e = dot2<double>(c, rhi, rhi, nullptr, nreal, st, c->sc + 8)) != cudaSuccess) return e;
+    if ((e = sc_read(c, 16, st)) != cudaSuccess) return e;
+    *rn = std::sqrt(c->sc_host[8]);
     return cudaSuccess;
   };
   if (bnorm == 0.0) {  // R15: b = 0 -> x = 0
     SOLVE_CUDA(cudaMemsetAsync(x_abi, 0, sizeof(double) * nreal, st));
     stt->converged = 1;
   } else {
-    double rnorm = 0, maxr, rz = 0, alpha = 0, beta = 0;
+    double rnorm = 0, maxr;
     SOLVE_CUDA(true_residual(&rnorm));                       // r0 = b - A x0 (R15)
     // fp16 sloppy vectors are kept in units of sigma ~ |r| at the last residual replacement (r_lo = r_hi / sigma, so
     // x_lo = x_true / sigma, p likewise): alpha and beta are scale invariant, and fp16 never underflows as r shrinks.
@@ -779,55 +779,76 @@ int solve_impl(mspcg_ctx* c, const double* b_abi, double* x_abi, const mspcg_sol
     else {
       if (prm->use_precond) { SOLVE_CUDA(precond_any(c, rlo, z, sp, prm->n_inner, prm->use_reduced_ls != 0, st)); stt->inner_applies += (long)prm->n_inner * c->lat.nblk; }
       SOLVE_CUDA(cudaMemcpyAsync(p, z, sizeof(TS) * nreal, cudaMemcpyDeviceToDevice, st));   // p0 = z0
-      SOLVE_CUDA(sc_zero(c, 2, st));
-      SOLVE_CUDA(dot2<TS>(c, rlo, z, nullptr, nreal, st));
-      SOLVE_CUDA(sc_read(c, 1, st));
-      rz = c->sc_host[0];
+      SOLVE_CUDA(sc_zero(c, SC_N, st));
+      SOLVE_CUDA(dot2<TS>(c, rlo, z, nullptr, nreal, st, c->sc + SC_RZN));
     }
-    while (!stt->converged && k < prm->max_iter) {
-      // Ap = A p; for k > 0 the update p = z + beta p is fused into kernel 1
-      MphiArgs<TS> mp; memset(&mp, 0, sizeof(mp));
-      if (k == 0) { mp.in = p; mp.mode = 0; } else { mp.in = z; mp.p = p; mp.mode = 1; mp.beta = beta; }
-      SOLVE_CUDA(sc_zero(c, 4, st));
-      SOLVE_CUDA(normal_full<TS>(c, obS, p, Ap, mp, c->sc, st));
-      stt->outer_applies++;
-      { const long nchunk = nreal / ST<TS>::PER;              // alpha_k = <r_k,z_k>/<p_k,A p_k> is formed on the device
-        k_outer_update<TS><<<(unsigned)((nchunk + 255) / 256), 256, 0, st>>>(p, Ap, rlo, xlo, nchunk, rz, c->sc, c->sc + 1);
-        c->launches++; }
-      SOLVE_CUDA(sc_read(c, 2, st));
-      const double pAp = c->sc_host[0];
-      if (!(pAp > 0.0)) { stt->breakdown = 1; rc = MSPCG_EBREAKDOWN; break; }   // the update kernel used alpha = 0
-      alpha = rz / pAp;
-      rnorm = std::sqrt(c->sc_host[1]) * sigma;
-      k++;
-      if (prm->history && k <= prm->history_len) prm->history[k - 1] = rnorm / bnorm;
-      if (!(rnorm == rnorm)) { stt->breakdown = 1; rc = MSPCG_EBREAKDOWN; break; }
-      bool replaced = false;
+    // The loop keeps <z,r>, alpha and beta in device memory (k_outer_update, k_outer_scalars): no kernel waits for the host.  The host
+    // reads (<p,Ap>, |r|^2) of iteration k - 1 from a pinned ring, written by the last kernel of that iteration, after it has queued
+    // iteration k: convergence and the reliable-update rule (R17) are evaluated one iteration late, and the GPU never idles.
+    constexpr int RING = 8;
+    double* ring = c->sc_host + 16;
+    cudaEvent_t evs[RING];
+    for (int i = 0; i < RING; i++) SOLVE_CUDA(cudaEventCreateWithFlags(&evs[i], cudaEventDisableTiming));
+    const bool self_z = !prm->use_precond;
+    int ignore_upto = 0;             // snapshots of iterations <= this were taken before the last residual replacement
+    auto replace_residual = [&]() -> int {   // R17 residual replacement / R15 confirmation with the true residual, then z, <z,r>, beta anew
+      SOLVE_CUDA(convert_any(c, xlo, sp, t64, 8, Vh, Ls, st));
+      SOLVE_CUDA(axpby<double>(c, sigma, t64, 1.0, xhi, nreal, st));
+      SOLVE_CUDA(cudaMemsetAsync(xlo, 0, sizeof(TS) * nreal, st));
+      SOLVE_CUDA(true_residual(&rnorm));
+      double f2 = 1.0;
+      if (rescale && rnorm > 0) {   // new unit: p keeps its true size, <z,r> follows
+        const double f = sigma / (rnorm * unit);
+        SOLVE_CUDA(axpby<TS>(c, 0.0, p, f, p, nreal, st));
+        f2 = f * f; sigma = rnorm * unit;
+      }
+      SOLVE_CUDA(convert_any(c, rhi, 8, rlo, sp, Vh, Ls, st, 1.0 / sigma));
+      maxr = rnorm; stt->reliable_updates++;
+      if (rnorm <= prm->tol * bnorm) { stt->converged = 1; return MSPCG_OK; }
+      if (prm->use_precond) { SOLVE_CUDA(precond_any(c, rlo, z, sp, prm->n_inner, prm->use_reduced_ls != 0, st)); stt->inner_applies += (long)prm->n_inner * c->lat.nblk; }
+      SOLVE_CUDA(dot2<TS>(c, z, rlo, nullptr, nreal, st, c->sc + SC_RZN));
+      k_outer_scalars<<<1, 1, 0, st>>>(c->sc, nullptr, 2, f2); c->launches++;
+      return MSPCG_OK;
+    };
+    auto handle = [&](int it) -> int {   // look at the snapshot of iteration `it` (1-based)
+      SOLVE_CUDA(cudaEventSynchronize(evs[it % RING]));
+      const double pAp = ring[2 * (it % RING)], rr = ring[2 * (it % RING) + 1];
+      const double rn = std::sqrt(rr) * sigma;
+      if (it > ignore_upto) {
+        if (!(pAp > 0.0) || !(rn == rn)) { stt->breakdown = 1; rc = MSPCG_EBREAKDOWN; return MSPCG_OK; }   // the update kernel used alpha = 0
+        rnorm = rn;
+      }
+      if (prm->history && it <= prm->history_len) prm->history[it - 1] = rn / bnorm;
+      if (it <= ignore_upto) return MSPCG_OK;
       if (rnorm <= prm->tol * bnorm || (sloppy && rnorm < prm->delta * maxr)) {
-        // R17 residual replacement / R15 confirmation with the true residual
-        SOLVE_CUDA(convert_any(c, xlo, sp, t64, 8, Vh, Ls, st));
-        SOLVE_CUDA(axpby<double>(c, sigma, t64, 1.0, xhi, nreal, st));
-        SOLVE_CUDA(cudaMemsetAsync(xlo, 0, sizeof(TS) * nreal, st));
-        SOLVE_CUDA(true_residual(&rnorm));
-        if (rescale && rnorm > 0) {   // new unit: p keeps its true size, <z,r> follows
-          const double f = sigma / (rnorm * unit);
-          SOLVE_CUDA(axpby<TS>(c, 0.0, p, f, p, nreal, st));
-          rz *= f * f; sigma = rnorm * unit;
-        }
-        SOLVE_CUDA(convert_any(c, rhi, 8, rlo, sp, Vh, Ls, st, 1.0 / sigma));
-        maxr = rnorm; stt->reliable_updates++; replaced = true;
-        if (rnorm <= prm->tol * bnorm) { stt->converged = 1; break; }
+        ignore_upto = k;
+        return replace_residual();
       }
       if (rnorm > maxr) maxr = rnorm;
-      if (prm->use_precond) { SOLVE_CUDA(precond_any(c, rlo, z, sp, prm->n_inner, prm->use_reduced_ls != 0, st)); stt->inner_applies += (long)prm->n_inner * c->lat.nblk; }
-      SOLVE_CUDA(sc_zero(c, 2, st));
-      SOLVE_CUDA(dot2<TS>(c, z, rlo, Ap, nreal, st));
-      SOLVE_CUDA(sc_read(c, 2, st));
-      const double rz_new = c->sc_host[0], zAp = c->sc_host[1];
-      // eq. 18: <z', r' - r>/<z, r> with r' - r = -alpha A p; Alg. 1's ratio right after a replacement (R16)
-      beta = replaced ? rz_new / rz : -alpha * zAp / rz;
-      rz = rz_new;
+      return MSPCG_OK;
+    };
+    int handled = 0;
+    if (!stt->converged) { k_outer_scalars<<<1, 1, 0, st>>>(c->sc, nullptr, 3, 1.0); c->launches++; }
+    while (!stt->converged && rc == MSPCG_OK && k < prm->max_iter) {
+      // Ap = A p; for k > 0 the update p = z + beta p is fused into kernel 1 (beta read from device memory)
+      MphiArgs<TS> mp; memset(&mp, 0, sizeof(mp));
+      if (k == 0) { mp.in = p; mp.mode = 0; } else { mp.in = z; mp.p = p; mp.mode = 1; mp.beta_dev = c->sc + SC_BETA; }
+      SOLVE_CUDA(normal_full<TS>(c, obS, p, Ap, mp, c->sc + SC_PAP, st));
+      stt->outer_applies++;
+      { const long nchunk = nreal / ST<TS>::PER;              // alpha_k = <r_k,z_k>/<p_k,A p_k> is formed on the device
+        k_outer_update<TS><<<(unsigned)((nchunk + 255) / 256), 256, 0, st>>>(p, Ap, rlo, xlo, nchunk, c->sc, self_z ? 1 : 0);
+        c->launches++; }
+      k++;
+      if (prm->use_precond) {
+        SOLVE_CUDA(precond_any(c, rlo, z, sp, prm->n_inner, prm->use_reduced_ls != 0, st)); stt->inner_applies += (long)prm->n_inner * c->lat.nblk;
+        SOLVE_CUDA(dot2<TS>(c, z, rlo, Ap, nreal, st, c->sc + SC_RZN));
+      }
+      k_outer_scalars<<<1, 1, 0, st>>>(c->sc, ring + 2 * (k % RING), 0, 1.0); c->launches++;   // eq. 18; snapshot for the host
+      SOLVE_CUDA(cudaEventRecord(evs[k % RING], st));
+      while (handled < k - 1 && !stt->converged && rc == MSPCG_OK) { handled++; int r_ = handle(handled); if (r_) return r_; }
     }
+    while (handled < k && !stt->converged && rc == MSPCG_OK) { handled++; int r_ = handle(handled); if (r_) return r_; }
+    for (int i = 0; i < RING; i++) cudaEventDestroy(evs[i]);
     if (!stt->converged && rc == MSPCG_OK) rc = MSPCG_ENOCONV;
     // x = x_hi + sigma x_lo, true residual, unpack
     SOLVE_CUDA(convert_any(c, xlo, sp, t64, 8, Vh, Ls, st));
@@ -1041,7 +1062,7 @@ int mspcg_set_workspace(mspcg_ctx* ctx, void* workspace_dev, size_t bytes, void*
     CUDA_OK(ctx, upload_frags(ctx->mfr_hat, ctx->hm_hat, ctx->Ls_hat, st));
     { int rc_ = upload_T(ctx, st); if (rc_) return rc_; }
   }
-  if (!ctx->sc_host) CUDA_OK(ctx, cudaMallocHost(&ctx->sc_host, sizeof(double) * 16));
+  if (!ctx->sc_host) CUDA_OK(ctx, cudaMallocHost(&ctx->sc_host, sizeof(double) * 64));
   { int dev = 0, n = 0;
     if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0) ctx->num_sms = n; }
   ctx->have_ws = true;
