@@ -48,13 +48,15 @@ def stage_sites(geo, full):
     return dict(nblk=geo["nblk"], nE0=geo["nE0"], nO=geo["nO1"], nE=geo["nE2"])
 
 
-def flops_normal(st, Ls):
-    """Flops of one D^dag D (or A_s, all blocks) application; SURVEY 8(d) convention."""
+def flops_normal(st, Ls, executed=False):
+    """Flops of one D^dag D (or A_s, all blocks) application; SURVEY 8(d) convention.  executed=True: what the library runs --
+    on the halo sites of a Dirichlet block kernel 3 applies the product matrix M5^-dag M5^-1 as ONE contraction and has no
+    xpay operand, so one contraction and the xpay are not executed there."""
     hop, bid, xpay, dense = 1320, 72, 48, 48 * Ls
-    # (SURVEY 8(d) convention: kernel 3 counts two contractions and the xpay on every site of its list, although the library
-    # applies the product matrix M5^-dag M5^-1 as one contraction on the halo sites of a Dirichlet block)
     per_block = (bid * st["nE0"] + (hop + dense) * st["nO"] + (hop + 2 * dense + xpay) * st["nE"]
                  + (hop + dense) * st["nO"] + (hop + bid + xpay) * st["nE0"]) * Ls
+    if executed:
+        per_block -= (dense + xpay) * (st["nE"] - st["nE0"]) * Ls
     return per_block * st["nblk"]
 
 
@@ -72,10 +74,10 @@ def bytes_normal(st, Ls, w, ng, fused_pupdate=False, with_dot=False):
     return dict(mphi=k1 * n, hop_k2=k2 * n, hop_k3=k3 * n, hop_k4=k4 * n, hop_k5=k5 * n)
 
 
-def precond_work(geo, Ls, k, w_in, w_io, ng):
+def precond_work(geo, Ls, k, w_in, w_io, ng, executed=False):
     """Flops and algorithmic bytes of one M^-1 application (k inner iterations)."""
     st = stage_sites(geo, False)
-    fl = k * flops_normal(st, Ls)
+    fl = k * flops_normal(st, Ls, executed)
     by = 0
     for it in range(k):
         b = bytes_normal(st, Ls, w_in, ng, fused_pupdate=it > 0, with_dot=True)
@@ -242,6 +244,7 @@ def run_ours(args):
     fl_op = flops_normal(st_full, Ls)
     by_op = sum(bytes_normal(st_full, Ls, 4, args.recon).values())
     flops_step = fl_pre + fl_op
+    flops_exec = precond_work(geo, Ls, k, 2, 4, args.recon, executed=True)[0] + fl_op
 
     # ---- the timed region (device-resident inputs)
     sampler = ClockSampler(local)
@@ -317,12 +320,13 @@ def run_ours(args):
                                     f"M_pre(k={k}, fp16 storage/fp32 math) + DdagD(fp32)" + (f" [reduced-Ls {args.reduced}: flop model of the full-Ls step, not a headline]" if args.reduced else ""),
                            parallelism="replicas only",
                            l2="working set of a step %.0f MiB > 126 MB L2 (no flush)" % (ws / 2**20), workspace_bytes=ws,
-                           flops_per_step=flops_step, alg_bytes_per_step=by_pre + by_op),
+                           flops_per_step=flops_step, flops_executed_per_step=flops_exec, alg_bytes_per_step=by_pre + by_op),
+               value_flops_executed=aggregate_value(flops_exec, ms_step, world),
                gpu_launches=launches, clocks=clocks, e2e=e2e, roofline=roofline, kernels=kern,
                step_GBps_algorithmic=(by_pre + by_op) / (ms_step * 1e-3) / 1e9)
     if rank == 0 and world == 1 and not args.no_extras and not big:
         out["extras"] = extras(torch, g, cfg, U, src, d_src, geo, peak, args)
-        out["cpu_baseline"] = cpu_baseline(cfg, U, src, geo)
+        out["cpu_baseline"] = cpu_baseline(cfg, U, src, geo, args.workload)
     if rank == 0:
         print(json.dumps(out))
     if world > 1:
@@ -455,26 +459,74 @@ def oracle_sample(cfg, U, src, geo):
     return run, flops, ora
 
 
-def cpu_baseline(cfg, U, src, geo):
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def cpu_baseline(cfg, U, src, geo, workload):
+    """The oracle as it stands on the host cores: the bounded sample on all cores and on one core (a second process with
+    OMP_NUM_THREADS=1), and full CG / MSPCG time-to-solution on C1."""
     run, flops, ora = oracle_sample(cfg, U, src, geo)
     t0 = time.time()
     run()
     dt = time.time() - t0
-    return dict(value=flops / dt / 1e9, unit=UNIT, cores=ora.threads, kind="oracle", seconds=dt,
-                sample="oracle M_pre on 1 of %d blocks (k=%d) + 1 full-lattice DdagD, fp64, same lattice" % (geo["nblk"], cfg["n_inner"]))
+    out = dict(value=flops / dt / 1e9, unit=UNIT, cores=ora.threads, kind="oracle", seconds=dt, cpu_model=cpu_model(),
+               sample="oracle M_pre on 1 of %d blocks (k=%d) + 1 full-lattice DdagD, fp64, same lattice" % (geo["nblk"], cfg["n_inner"]))
+    try:   # one core: the same sample in a fresh process (the OpenMP thread count is fixed at library load)
+        env = dict(os.environ, OMP_NUM_THREADS="1")
+        res = subprocess.run([sys.executable, os.path.abspath(__file__), "--impl", "reference", "--steps", "1", "--warmup", "0",
+                              "--workload", workload], env=env, capture_output=True, text=True, timeout=600)
+        one = json.loads(res.stdout.strip().splitlines()[-1])
+        out["value_1core"] = one["value"]
+        out["seconds_1core"] = one["ms_per_step"] * 1e-3
+    except Exception as e:   # noqa: BLE001
+        out["value_1core"] = None
+        out["note_1core"] = "one-core run failed: %r" % (e,)
+    out["C1_time_to_solution"] = oracle_solves("C1")
+    return out
+
+
+def oracle_solves(workload):
+    """Full CG and MSPCG solves to 1e-10 on the CPU oracle (fp64 throughout): seconds, outer iterations, inner applications."""
+    from oracle.cbind import OracleC
+    cfg = synth.CONFIGS[workload]
+    U, src = make_inputs(cfg)
+    ora = OracleC(cfg["dims"], cfg["Ls"], cfg["b"], cfg["c"], cfg["M5"], cfg["mf"], cfg["block"])
+    ora.load_gauge(U, -1)
+    res = dict(lattice=list(cfg["dims"]), Ls=cfg["Ls"], block=list(cfg["block"]), n_inner=cfg["n_inner"], cores=ora.threads)
+    for name, pre in (("CG", False), ("MSPCG", True)):
+        t0 = time.time()
+        _, st = ora.solve(src, tol=1e-10, use_precond=pre, n_inner=cfg["n_inner"])
+        res[name] = dict(seconds=time.time() - t0, outer_iters=st["iters"], inner_applies=st["inner_applies"], true_res=st["true_res"], rc=st["rc"])
+    return res
 
 
 def host_geometry(cfg):
-    from paper_2104_05615_b200 import Mspcg
-    m = Mspcg(cfg["dims"], cfg["Ls"], cfg["b"], cfg["c"], cfg["M5"], cfg["mf"], cfg["block"])
-    geo = m.geometry()
-    m.close()
-    return geo
+    """Site counts of the stage lists of one Dirichlet block (pad of two, L1 overshoot d; even d<=2, odd d<=1),
+    counted here with numpy so that the oracle arm loads nothing of the product library."""
+    dims, block = cfg["dims"], cfg["block"]
+    cut = [b != l for b, l in zip(block, dims)]
+    axes = [np.arange(-2, b + 2) if c else np.arange(0, b) for b, c in zip(block, cut)]
+    X = np.meshgrid(*axes, indexing="ij")
+    d = sum(((-x).clip(0) + (x - (b - 1)).clip(0)) if c else 0 * x for x, b, c in zip(X, block, cut))
+    par = sum(X) % 2
+    nblk = int(np.prod([l // b for l, b in zip(dims, block)]))
+    return dict(nblk=nblk, nE0=int(((par == 0) & (d == 0)).sum()), nE2=int(((par == 0) & (d <= 2)).sum()),
+                nO1=int(((par == 1) & (d <= 1)).sum()), vh=int(np.prod(dims)) // 2)
 
 
 def run_reference(args):
     """The reference arm of this tier is the CPU oracle, as it stands, on the box's host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
+        return
+    if args.cpu_solves:   # BASELINE.md section 4: full oracle solves on a lattice that finishes in minutes
+        print(json.dumps(dict(impl="reference", cpu_model=cpu_model(), time_to_solution=oracle_solves(args.cpu_solves))))
         return
     cfg = synth.CONFIGS[args.workload]
     U, src = make_inputs(cfg)
@@ -496,7 +548,7 @@ def run_reference(args):
         config=dict(workload=f"{args.workload}: {dims[0]}x{dims[1]}x{dims[2]}x{dims[3]} Ls={Ls} blocks {block} (bounded sample)",
                     parallelism="host cores"),
         gpu_launches=0,
-        cpu_baseline=dict(value=val, unit=UNIT, cores=ora.threads, kind="oracle", sample=sample),
+        cpu_baseline=dict(value=val, unit=UNIT, cores=ora.threads, kind="oracle", sample=sample, cpu_model=cpu_model()),
         e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))))
 
 
@@ -512,6 +564,7 @@ def main():
     ap.add_argument("--recon", type=int, default=18, choices=[12, 18], help="link storage of the low-precision copies (12 = two rows, R8)")
     ap.add_argument("--train-steps", type=int, default=100, help="line-search steps of the T training in the extras")
     ap.add_argument("--mu", type=float, default=0.85, help="shift mu of the reduced-Ls preconditioner in the extras (PAPER.md:309 eq. 20; the paper's tuned values: 0.437-0.85)")
+    ap.add_argument("--cpu-solves", default="", choices=["", "C1", "C3p"], help="with --impl reference: full CG and MSPCG solves on the CPU oracle on this lattice (C3p = reduced C3: 12^3 x 24, Ls 8)")
     ap.add_argument("--reduced", type=int, default=0, help="profiling aid: run the step with the reduced-Ls preconditioner at this Ls_hat")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -175,6 +175,13 @@ typedef struct {
 int mspcg_solve(mspcg_ctx* ctx, const double* b_dev, double* x_dev, const mspcg_solve_params* params,
                 mspcg_solve_stats* stats, void* stream);
 
+/* r = b - D^dag D x in fp64 (the true residual of PAPER.md:117 eq. 9; the training vectors of PAPER.md:322 are such residuals of
+ * a full-Ls MSPCG run).  b_dev, x_dev, r_dev: DEVICE fp64 ABI vectors; r_dev may not alias b_dev or x_dev.  normalise != 0:
+ * r is divided by |r|_2 (left as is when r = 0).  *rnorm_host (HOST, may be NULL) receives |b - D^dag D x|_2.  Synchronous.
+ * Uses the solver's vectors as scratch.  Errors: MSPCG_EINVAL (null pointer, aliasing), MSPCG_ENOGAUGE / MSPCG_ENOWORKSPACE. */
+int mspcg_residual(mspcg_ctx* ctx, const double* b_dev, const double* x_dev, double* r_dev, int normalise, double* rnorm_host,
+                   void* stream);
+
 /* Counters for reports: kernels launched by this context since creation. */
 long mspcg_launch_count(const mspcg_ctx* ctx);
 

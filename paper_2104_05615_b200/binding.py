@@ -24,7 +24,7 @@ SYMBOLS = [
     "mspcg_unpack", "mspcg_apply_MdagM", "mspcg_apply_precond", "mspcg_apply_MdagM_host",
     "mspcg_apply_precond_host", "mspcg_apply_A_block", "mspcg_set_reduced_ls", "mspcg_solve", "mspcg_launch_count",
     "mspcg_timing", "mspcg_timing_read", "mspcg_update_T", "mspcg_train_eval", "mspcg_train_T",
-    "mspcg_prepare_source", "mspcg_reconstruct_odd", "mspcg_apply_full", "mspcg_apply_M5inv",
+    "mspcg_prepare_source", "mspcg_reconstruct_odd", "mspcg_apply_full", "mspcg_apply_M5inv", "mspcg_residual",
 ]
 
 
@@ -74,6 +74,7 @@ def load_library():
     L.mspcg_prepare_source.argtypes = [vp, vp, vp, vp, vp, vp]
     L.mspcg_reconstruct_odd.argtypes = [vp, vp, vp, vp, vp]
     L.mspcg_apply_full.argtypes = [vp, vp, vp, vp, vp, vp]
+    L.mspcg_residual.argtypes = [vp, vp, vp, vp, i, dp, vp]
     L.mspcg_set_reduced_ls.argtypes = [vp, i, dp, d]
     L.mspcg_solve.argtypes = [vp, vp, vp, C.POINTER(SolveParams), C.POINTER(SolveStats), vp]
     L.mspcg_launch_count.argtypes = [vp]
@@ -274,6 +275,15 @@ class Mspcg:
         self._check(self.lib.mspcg_apply_full(self.h, C.c_void_p(psi_e_abi.data_ptr()), C.c_void_p(psi_o_abi.data_ptr()),
                                               C.c_void_p(oe.data_ptr()), C.c_void_p(oo.data_ptr()), self._stream()))
         return oe, oo
+
+    def residual(self, b_abi, x_abi, normalise=False):
+        """r = b - D^dag D x in fp64 (mspcg_residual), optionally divided by its norm; returns (r, |b - D^dag D x|)."""
+        torch = _torch()
+        r = torch.empty_like(b_abi)
+        rn = C.c_double()
+        self._check(self.lib.mspcg_residual(self.h, C.c_void_p(b_abi.data_ptr()), C.c_void_p(x_abi.data_ptr()), C.c_void_p(r.data_ptr()),
+                                            int(bool(normalise)), C.byref(rn), self._stream()))
+        return r, rn.value
 
     def apply_MdagM_host(self, v_host, out_host, prec=F64):
         self._check(self.lib.mspcg_apply_MdagM_host(self.h, C.c_void_p(v_host.data_ptr()), C.c_void_p(out_host.data_ptr()), prec))

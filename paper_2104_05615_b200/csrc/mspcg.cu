@@ -1235,6 +1235,28 @@ int mspcg_solve(mspcg_ctx* ctx, const double* b_dev, double* x_dev, const mspcg_
   return solve_impl<__half>(ctx, b_dev, x_dev, params, stats, st);
 }
 
+int mspcg_residual(mspcg_ctx* ctx, const double* b_dev, const double* x_dev, double* r_dev, int normalise, double* rnorm_host, void* stream) {
+  int rc = check_ready(ctx, true); if (rc) return rc;
+  if (!b_dev || !x_dev || !r_dev || r_dev == b_dev || r_dev == x_dev) return fail(ctx, MSPCG_EINVAL, "null pointer or aliasing");
+  cudaStream_t st = (cudaStream_t)stream;
+  const long nreal = v5h(ctx, ctx->Ls) * 24;
+  double *b = ctx->v_b, *x = ctx->v_xhi, *r = ctx->v_rhi, *t = ctx->v_t64;
+  CUDA_OK(ctx, pack_any(ctx, b_dev, b, MSPCG_F64, 1, st));
+  CUDA_OK(ctx, pack_any(ctx, x_dev, x, MSPCG_F64, 1, st));
+  CUDA_OK(ctx, normal_full<double>(ctx, ctx->full64, x, t, mphi_plain<double>(x), nullptr, st));
+  CUDA_OK(ctx, cudaMemcpyAsync(r, b, sizeof(double) * nreal, cudaMemcpyDeviceToDevice, st));
+  CUDA_OK(ctx, axpby<double>(ctx, -1.0, t, 1.0, r, nreal, st));
+  CUDA_OK(ctx, cudaMemsetAsync(ctx->sc + 8, 0, sizeof(double), st));
+  CUDA_OK(ctx, dot2<double>(ctx, r, r, nullptr, nreal, st, ctx->sc + 8));
+  CUDA_OK(ctx, sc_read(ctx, 16, st));
+  const double rn = std::sqrt(ctx->sc_host[8]);
+  if (rnorm_host) *rnorm_host = rn;
+  if (normalise && rn > 0.0) CUDA_OK(ctx, axpby<double>(ctx, 0.0, r, 1.0 / rn, r, nreal, st));
+  CUDA_OK(ctx, pack_any(ctx, r_dev, r, MSPCG_F64, 0, st));
+  CUDA_OK(ctx, cudaStreamSynchronize(st));
+  return MSPCG_OK;
+}
+
 int mspcg_update_T(mspcg_ctx* ctx, const double* T_host, double mu, void* stream) {
   int rc = check_ready(ctx, false); if (rc) return rc;
   if (!ctx->Ls_hat || !T_host) return fail(ctx, MSPCG_EINVAL, "mspcg_update_T needs mspcg_set_reduced_ls before the workspace was sized");

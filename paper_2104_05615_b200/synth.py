@@ -147,4 +147,7 @@ CONFIGS = {
                block=(16, 16, 16, 32), n_inner=6, Ls_hat=6, **MOBIUS),
     "C5": dict(dims=(48, 48, 48, 96), Ls=12, mf=0.001, eps=0.1, gauge_seed=15, src_seed=25,
                block=(8, 8, 8, 8), n_inner=6, **MOBIUS),
+    # reduced C3 (SURVEY 8(d) CPU baseline plan): same parameters on a lattice the CPU oracle solves in minutes
+    "C3p": dict(dims=(12, 12, 12, 24), Ls=8, mf=0.002, eps=0.1, gauge_seed=13, src_seed=2,
+                block=(6, 6, 6, 12), n_inner=5, **MOBIUS),
 }

@@ -27,14 +27,13 @@ def initial_T_abi(Ls, Lh):
 
 
 def residual_vectors(g, d_b, n_inner, n_vec, span):
-    """r_k = b - A x_k of a full-Ls MSPCG run (fp64 operator), k = span/n_vec, 2 span/n_vec, ...; normalised."""
+    """r_k = b - A x_k of a full-Ls MSPCG run (fp64 operator), k = span/n_vec, 2 span/n_vec, ...; normalised.  torch only concatenates."""
     import torch
     out = []
     for j in range(1, n_vec + 1):
         k = max(1, (span * j) // n_vec)
         x, _ = g.solve(d_b, tol=1e-14, max_iter=k, use_precond=True, n_inner=n_inner, sloppy_prec=F32)
-        r = d_b - g.apply_MdagM(x, F64)
-        out.append(r / torch.linalg.vector_norm(r))
+        out.append(g.residual(d_b, x, normalise=True)[0])   # formed and normalised inside the library (mspcg_residual)
     return torch.cat(out)
 
 

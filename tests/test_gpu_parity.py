@@ -179,8 +179,10 @@ def test_solve_C1_cg_and_mspcg_fp64():
         assert rel(ora.apply_MdagM(xn), b) <= 1e-10 * 1.01
         assert rel(xn, x_ora) <= 1e-8
     assert rel(x_orap, x_ora) <= 1e-8
-    assert abs(s["iters"] - so["iters"]) <= 3
-    assert abs(spc["iters"] - sop["iters"]) <= 3
+    # iteration counts against the oracle's (eq. 18 beta on both sides): the library looks at |r| one iteration late (R15b),
+    # so it may run one iteration more; rounding order accounts for the other one
+    assert abs(s["iters"] - so["iters"]) <= 2, (s["iters"], so["iters"])
+    assert abs(spc["iters"] - sop["iters"]) <= 2, (spc["iters"], sop["iters"])
     assert spc["iters"] < s["iters"]
     assert spc["inner_applies"] > 0
 
