@@ -224,6 +224,7 @@ def run_ours(args):
     if args.reduced:   # profiling aid: the step's preconditioner becomes the reduced-Ls one (untrained T, eq. 20-21)
         g.set_reduced_ls(args.reduced, initial_T_abi(Ls, args.reduced), 0.5)
     ws = g.configure(F32, F16, args.recon)
+    g.set_block_group(args.group)
     g.load_gauge(U, -1)
     geo = g.geometry()
     d_src = torch.as_tensor(src.reshape(-1)).cuda()
@@ -318,7 +319,7 @@ def run_ours(args):
                data="synthetic", impl="ours",
                config=dict(workload=f"{args.workload}: {dims[0]}x{dims[1]}x{dims[2]}x{dims[3]} Ls={Ls} blocks {block} "
                                     f"M_pre(k={k}, fp16 storage/fp32 math) + DdagD(fp32)" + (f" [reduced-Ls {args.reduced}: flop model of the full-Ls step, not a headline]" if args.reduced else ""),
-                           parallelism="replicas only",
+                           parallelism="replicas only", block_group=args.group,
                            l2="working set of a step %.0f MiB > 126 MB L2 (no flush)" % (ws / 2**20), workspace_bytes=ws,
                            flops_per_step=flops_step, flops_executed_per_step=flops_exec, alg_bytes_per_step=by_pre + by_op),
                value_flops_executed=aggregate_value(flops_exec, ms_step, world),
@@ -364,8 +365,7 @@ def extras(torch, g, cfg, U, src, d_src, geo, peak, args):
     sol = {}
     for name, pre in (("CG", False), ("MSPCG", True)):
         x, s = g.solve(d_src, tol=1e-10, max_iter=200000, use_precond=pre, n_inner=k, sloppy_prec=F32, delta=0.1)
-        sol[name] = dict(seconds=s["seconds"], outer_iters=s["iters"], reliable_updates=s["reliable_updates"],
-                         inner_applies=s["inner_applies"], true_res=s["true_res"], rc=s["rc"])
+        sol[name] = solve_entry(s)
     ex["solve_tol1e-10_fp32outer_fp16inner"] = sol
     del x
     g.close()
@@ -375,20 +375,8 @@ def extras(torch, g, cfg, U, src, d_src, geo, peak, args):
     # T is the identity in 4D site and colour (eq. 21), so it is trained on a sample lattice of at most 16^3 x 32 sites with the same
     # Moebius parameters, mass and link roughness (its own seeds) and Dirichlet blocks of at most half its extent, and then
     # used on the full lattice -- the paper likewise trains once per ensemble.
-    from paper_2104_05615_b200.train_reduced_ls import train
     Lh, mu = cfg.get("Ls_hat", Ls // 2), args.mu
-    tdims = tuple(min(d, 16 if i < 3 else 32) for i, d in enumerate(dims))
-    tblock = tuple(min(b, t // 2) if b < d else t for b, t, d in zip(block, tdims, dims))
-    if tdims == tuple(dims):
-        U_t, src_t, tblock = U, src, block
-    else:
-        U_t = synth.gauge_natural_to_abi(synth.random_su3_links(tdims, cfg["eps"], cfg["gauge_seed"] + 100), tdims)
-        src_t = synth.gaussian_spinor_abi(tdims, Ls, cfg["src_seed"] + 100)
-    t0 = time.time()
-    T, info = train(tdims, Ls, dict(b=cfg["b"], c=cfg["c"], M5=cfg["M5"]), cfg["mf"], tblock, U_t, src_t, Lh, mu, k,
-                    n_vec=12, span=120, n_steps=args.train_steps, momentum=0.5)
-    torch.cuda.synchronize()
-    train_s = time.time() - t0
+    T, info, train_s, tdims, tblock = train_T_on_sample(torch, cfg, U, src, args)
     gr = Mspcg(dims, Ls, cfg["b"], cfg["c"], cfg["M5"], cfg["mf"], block)
     gr.set_reduced_ls(Lh, T, mu)
     gr.configure(F32, F16, 18)
@@ -398,8 +386,7 @@ def extras(torch, g, cfg, U, src, d_src, geo, peak, args):
     x, s = gr.solve(d_src, tol=1e-10, max_iter=200000, use_precond=True, n_inner=k, sloppy_prec=F32, delta=0.1, use_reduced_ls=True)
     ex["reducedLs%d_trainedT_mu%.2f" % (Lh, mu)] = dict(
         Mpre_ms=ms, train_seconds=train_s, train_steps=args.train_steps, train_lattice=list(tdims), train_block=list(tblock), chi2_first=float(info["chi2"][0]), chi2_last=float(info["chi2"][-1]),
-        solve=dict(seconds=s["seconds"], outer_iters=s["iters"], reliable_updates=s["reliable_updates"],
-                   inner_applies=s["inner_applies"], true_res=s["true_res"], rc=s["rc"]))
+        solve=solve_entry(s))
     del x, v, o
     gr.close()
     torch.cuda.empty_cache()
@@ -435,12 +422,81 @@ def extras(torch, g, cfg, U, src, d_src, geo, peak, args):
     cap = 3 * ex["solve_tol1e-10_fp32outer_fp16inner"]["CG"]["outer_iters"]   # plain fp16 CG can stagnate on ill-conditioned systems (rc = ENOCONV then)
     for name, pre in (("CG", False), ("MSPCG", True)):
         x, s = g3.solve(d_src, tol=1e-10, max_iter=cap, use_precond=pre, n_inner=k, sloppy_prec=F16, delta=0.1)
-        sol[name] = dict(seconds=s["seconds"], outer_iters=s["iters"], reliable_updates=s["reliable_updates"],
-                         inner_applies=s["inner_applies"], true_res=s["true_res"], rc=s["rc"])
+        sol[name] = solve_entry(s)
     ex["solve_tol1e-10_fp16outer_fp16inner"] = sol
     del x
     g3.close()
     return ex
+
+
+def train_T_on_sample(torch, cfg, U, src, args):
+    """T of the reduced-Ls preconditioner (eq. 21) trained with the library (eq. 22) on a sample lattice of at most 16^3 x 32 sites with the
+    configuration's parameters (its own seeds; Dirichlet blocks at most half its extent); T is site and colour independent (R20)."""
+    from paper_2104_05615_b200.train_reduced_ls import train
+    dims, Ls, block, k = cfg["dims"], cfg["Ls"], cfg["block"], cfg["n_inner"]
+    Lh, mu = cfg.get("Ls_hat", Ls // 2), args.mu
+    tdims = tuple(min(d, 16 if i < 3 else 32) for i, d in enumerate(dims))
+    tblock = tuple(min(b, t // 2) if b < d else t for b, t, d in zip(block, tdims, dims))
+    if tdims == tuple(dims):
+        U_t, src_t, tblock = U, src, block
+    else:
+        U_t = synth.gauge_natural_to_abi(synth.random_su3_links(tdims, cfg["eps"], cfg["gauge_seed"] + 100), tdims)
+        src_t = synth.gaussian_spinor_abi(tdims, Ls, cfg["src_seed"] + 100)
+    t0 = time.time()
+    T, info = train(tdims, Ls, dict(b=cfg["b"], c=cfg["c"], M5=cfg["M5"]), cfg["mf"], tblock, U_t, src_t, Lh, mu, k,
+                    n_vec=12, span=120, n_steps=args.train_steps, momentum=0.5)
+    torch.cuda.synchronize()
+    return T, info, time.time() - t0, tdims, tblock
+
+
+def solve_entry(s):
+    return dict(seconds=s["seconds"], outer_iters=s["iters"], reliable_updates=s["reliable_updates"],
+                inner_applies=s["inner_applies"], outer_applies=s["outer_applies"], true_res=s["true_res"], rc=s["rc"])
+
+
+def run_solves(args):
+    """Time to solution on one GPU (BASELINE.json metric, Tables 3-4): plain CG, MSPCG and MSPCG with the reduced-Ls
+    preconditioner on the workload, sloppy outer precision --sloppy (fp32 or fp16) with fp64 residual replacement, fp16 preconditioner, 1e-10."""
+    import torch
+    from paper_2104_05615_b200 import F16, F32, Mspcg
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    cfg = dict(synth.CONFIGS[args.workload])
+    if args.block:
+        cfg["block"] = tuple(int(x) for x in args.block.split(","))
+    if args.n_inner:
+        cfg["n_inner"] = args.n_inner
+    dims, Ls, block, k = cfg["dims"], cfg["Ls"], cfg["block"], cfg["n_inner"]
+    sloppy = F16 if args.sloppy == 16 else F32
+    U, src = make_inputs(cfg)
+    out = dict(impl="ours", mode="solves", workload=args.workload, lattice=list(dims), Ls=Ls, block=list(block), n_inner=k, mf=cfg["mf"],
+               sloppy_bits=args.sloppy, recon=args.recon, tol=1e-10, solves={})
+    Lh = cfg.get("Ls_hat", Ls // 2)
+    T = None
+    if args.reduced_solve:
+        T, info, train_s, tdims, tblock = train_T_on_sample(torch, cfg, U, src, args)
+        out["reduced"] = dict(Ls_hat=Lh, mu=args.mu, train_seconds=train_s, train_steps=args.train_steps, train_lattice=list(tdims),
+                              train_block=list(tblock), chi2_first=float(info["chi2"][0]), chi2_last=float(info["chi2"][-1]))
+    g = Mspcg(dims, Ls, cfg["b"], cfg["c"], cfg["M5"], cfg["mf"], block)
+    if T is not None:
+        g.set_reduced_ls(Lh, T, args.mu)
+    out["workspace_bytes"] = g.configure(sloppy, F16, args.recon)
+    g.set_block_group(args.group)
+    out["block_group"] = args.group
+    g.load_gauge(U, -1)
+    del U
+    d_src = torch.as_tensor(src.reshape(-1)).cuda()
+    sampler = ClockSampler(int(os.environ.get("LOCAL_RANK", "0")))
+    sampler.start()
+    cap = args.max_iter
+    for name, kw in (("CG", dict(use_precond=False)), ("MSPCG", dict(use_precond=True, n_inner=k)),
+                     ("MSPCG_reducedLs", dict(use_precond=True, n_inner=k, use_reduced_ls=True))):
+        if name == "MSPCG_reducedLs" and T is None:
+            continue
+        x, st = g.solve(d_src, tol=1e-10, max_iter=cap, sloppy_prec=sloppy, delta=0.1, **kw)
+        del x
+        out["solves"][name] = solve_entry(st)
+    out["clocks"] = sampler.stop()
+    print(json.dumps(out))
 
 
 def oracle_sample(cfg, U, src, geo):
@@ -565,11 +621,19 @@ def main():
     ap.add_argument("--train-steps", type=int, default=100, help="line-search steps of the T training in the extras")
     ap.add_argument("--mu", type=float, default=0.85, help="shift mu of the reduced-Ls preconditioner in the extras (PAPER.md:309 eq. 20; the paper's tuned values: 0.437-0.85)")
     ap.add_argument("--cpu-solves", default="", choices=["", "C1", "C3p"], help="with --impl reference: full CG and MSPCG solves on the CPU oracle on this lattice (C3p = reduced C3: 12^3 x 24, Ls 8)")
+    ap.add_argument("--group", type=int, default=0, help="Dirichlet blocks per L2-resident group of the preconditioner (mspcg_set_block_group; 0 = all at once)")
+    ap.add_argument("--solves", action="store_true", help="time to solution instead of the step benchmark: CG, MSPCG (and reduced-Ls MSPCG with --reduced-solve) on --workload")
+    ap.add_argument("--reduced-solve", action="store_true", help="with --solves: also train T on a sample lattice and solve with the reduced-Ls preconditioner")
+    ap.add_argument("--sloppy", type=int, default=32, choices=[16, 32], help="with --solves: bits of the sloppy outer iteration")
+    ap.add_argument("--n-inner", type=int, default=0, help="with --solves: inner iterations (default: the configuration's)")
+    ap.add_argument("--max-iter", type=int, default=200000)
     ap.add_argument("--reduced", type=int, default=0, help="profiling aid: run the step with the reduced-Ls preconditioner at this Ls_hat")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
+    elif args.solves:
+        run_solves(args)
     else:
         run_ours(args)
 

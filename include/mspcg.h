@@ -182,6 +182,13 @@ int mspcg_solve(mspcg_ctx* ctx, const double* b_dev, double* x_dev, const mspcg_
 int mspcg_residual(mspcg_ctx* ctx, const double* b_dev, const double* x_dev, double* r_dev, int normalise, double* rnorm_host,
                    void* stream);
 
+/* Block-resident inner CG (preconditioner kernels are global-memory or L2 bound; blocks are
+ * independent).  blocks_per_group = G > 0: mspcg_apply_precond (and the preconditioner inside mspcg_solve) runs all inner iterations for G
+ * Dirichlet blocks at a time, reusing the same G-block buffers for every group, so that with G x (per-block working set) below the
+ * 126 MB L2 the inner vectors never travel to HBM.  0 (default): all blocks in one batch.  Results are identical (the blocks do not
+ * interact, R13).  The environment variable MSPCG_GROUP sets the default of new contexts.  Errors: MSPCG_EINVAL (G < 0). */
+int mspcg_set_block_group(mspcg_ctx* ctx, int blocks_per_group);
+
 /* Counters for reports: kernels launched by this context since creation. */
 long mspcg_launch_count(const mspcg_ctx* ctx);
 

@@ -12,7 +12,7 @@ import os
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libmspcg.so")
+LIB_PATH = os.environ.get("MSPCG_LIB", os.path.join(HERE, "libmspcg.so"))   # MSPCG_LIB: an alternative build (kernel experiments)
 
 F64, F32, F16 = 8, 4, 2
 LAYOUT_ABI, LAYOUT_NATIVE = 0, 1
@@ -24,7 +24,7 @@ SYMBOLS = [
     "mspcg_unpack", "mspcg_apply_MdagM", "mspcg_apply_precond", "mspcg_apply_MdagM_host",
     "mspcg_apply_precond_host", "mspcg_apply_A_block", "mspcg_set_reduced_ls", "mspcg_solve", "mspcg_launch_count",
     "mspcg_timing", "mspcg_timing_read", "mspcg_update_T", "mspcg_train_eval", "mspcg_train_T",
-    "mspcg_prepare_source", "mspcg_reconstruct_odd", "mspcg_apply_full", "mspcg_apply_M5inv", "mspcg_residual",
+    "mspcg_prepare_source", "mspcg_reconstruct_odd", "mspcg_apply_full", "mspcg_apply_M5inv", "mspcg_residual", "mspcg_set_block_group",
 ]
 
 
@@ -75,6 +75,7 @@ def load_library():
     L.mspcg_reconstruct_odd.argtypes = [vp, vp, vp, vp, vp]
     L.mspcg_apply_full.argtypes = [vp, vp, vp, vp, vp, vp]
     L.mspcg_residual.argtypes = [vp, vp, vp, vp, i, dp, vp]
+    L.mspcg_set_block_group.argtypes = [vp, i]
     L.mspcg_set_reduced_ls.argtypes = [vp, i, dp, d]
     L.mspcg_solve.argtypes = [vp, vp, vp, C.POINTER(SolveParams), C.POINTER(SolveStats), vp]
     L.mspcg_launch_count.argtypes = [vp]
@@ -275,6 +276,10 @@ class Mspcg:
         self._check(self.lib.mspcg_apply_full(self.h, C.c_void_p(psi_e_abi.data_ptr()), C.c_void_p(psi_o_abi.data_ptr()),
                                               C.c_void_p(oe.data_ptr()), C.c_void_p(oo.data_ptr()), self._stream()))
         return oe, oo
+
+    def set_block_group(self, blocks_per_group):
+        """L2-resident groups of Dirichlet blocks for the preconditioner (mspcg_set_block_group); 0 = all blocks at once."""
+        self._check(self.lib.mspcg_set_block_group(self.h, int(blocks_per_group)))
 
     def residual(self, b_abi, x_abi, normalise=False):
         """r = b - D^dag D x in fp64 (mspcg_residual), optionally divided by its norm; returns (r, |b - D^dag D x|)."""

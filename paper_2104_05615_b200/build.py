@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmspcg.so")
 SOURCES = ["mspcg.cu"]
-DEPS = ["mspcg.cu", "kernels.cuh", "hop_mma.cuh", "hop_tile.cuh", "tile_tables.hpp", "transfer_tc.cuh", "site_math.cuh", "geometry.hpp", os.path.join("..", "..", "include", "mspcg.h")]
+DEPS = ["mspcg.cu", "kernels.cuh", "hop_mma.cuh", "hop_tile.cuh", "tile_tables.hpp", "dense5d_tma.cuh", "transfer_tc.cuh", "site_math.cuh", "geometry.hpp", os.path.join("..", "..", "include", "mspcg.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
@@ -36,7 +36,9 @@ def up_to_date():
 def build(force=False, verbose=False):
     if not force and up_to_date():
         return LIB
-    cmd = [_nvcc()] + NVCC_FLAGS + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+    extra = os.environ.get("MSPCG_NVCC_EXTRA", "").split()   # experiments: -D switches
+    out = os.environ.get("MSPCG_LIB_OUT", LIB)
+    cmd = [_nvcc()] + NVCC_FLAGS + extra + ["-o", out] + [os.path.join(CSRC, s) for s in SOURCES]
     res = subprocess.run(cmd, capture_output=True, text=True)
     with open(os.path.join(HERE, "build.log"), "w") as f:
         f.write(" ".join(cmd) + "\n" + res.stdout + res.stderr)
@@ -44,8 +46,8 @@ def build(force=False, verbose=False):
         sys.stderr.write(res.stdout[-4000:] + res.stderr[-4000:])
         raise RuntimeError("nvcc failed building libmspcg.so")
     if verbose:
-        print(LIB)
-    return LIB
+        print(out)
+    return out
 
 
 if __name__ == "__main__":

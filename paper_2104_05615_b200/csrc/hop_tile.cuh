@@ -24,9 +24,17 @@
 
 namespace mspcg {
 
-template <int LS> struct TileCfg {
+#ifndef MSPCG_TILE_NWC_PLAIN
+#define MSPCG_TILE_NWC_PLAIN 16
+#endif
+#ifndef MSPCG_TILE_NWP_PLAIN
+#define MSPCG_TILE_NWP_PLAIN 4
+#endif
+template <int LS, int EPI = 0> struct TileCfg {
   enum {
-    TS = TILE_TS, NIN = TILE_NIN, NWC = 16, NWP = 4, NSTAGE = 2,   // consumer warps, producer warps, pipeline stages
+    TS = TILE_TS, NIN = TILE_NIN, NSTAGE = 2,
+    NWC = (EPI == 0 ? MSPCG_TILE_NWC_PLAIN : 16),   // consumer warps (the plain epilogue needs fewer registers: more warps fit)
+    NWP = (EPI == 0 ? MSPCG_TILE_NWP_PLAIN : 4),    // producer warps
     COL = LS * 48,                       // bytes of one site column
     LINKREC = 8 * 18 * 2,                // bytes of the eight links of one output site
     OFF_ZERO = NIN * COL,                // one column of zeros: the slot of every absent neighbour (and of the pad lanes' link words)
@@ -81,9 +89,9 @@ __device__ __forceinline__ void hop_mu_full(float (&S)[MmaCfg<LS>::NMT][4], cons
 }
 
 template <int LS, int EPI>
-__global__ void __launch_bounds__(TileCfg<LS>::THREADS, 1) k_hop_tile(const HopArgs<__half> a) {
+__global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const HopArgs<__half> a) {
   typedef MmaCfg<LS> Cfg;
-  typedef TileCfg<LS> TC;
+  typedef TileCfg<LS, EPI> TC;
   constexpr int NSEG = Cfg::NSEG, NMT = Cfg::NMT, NWC = TC::NWC;
   extern __shared__ __align__(128) unsigned char smraw[];
   __shared__ uint4 sfrag[(EPI == EPI_K3 ? 2 : 1) * 64];   // A fragments of the 5D matrices
@@ -182,7 +190,7 @@ __global__ void __launch_bounds__(TileCfg<LS>::THREADS, 1) k_hop_tile(const HopA
     }
     asm volatile("bar.sync 1, %0;\n" ::"n"(32 * NWC) : "memory");   // consumer warps only
   }
-  int blk = blk0, ti = ti0;
+  int blk = blk0, ti = ti0, rot = 0;
   for (long tt = t_begin; tt < t_end; tt++) {
     if (blk != part_blk) { flush_dot(); part_blk = blk; }
     const uint4* aux4 = nullptr; const uint4* dot4 = nullptr;
@@ -199,7 +207,8 @@ __global__ void __launch_bounds__(TileCfg<LS>::THREADS, 1) k_hop_tile(const HopA
     const uint32_t* lk32 = reinterpret_cast<const uint32_t*>(smraw + stage * TC::STAGE + TC::OFF_LINK);
     const uint32_t* zero32 = reinterpret_cast<const uint32_t*>(smraw + stage * TC::STAGE + TC::OFF_ZERO);
     const int n_out = (int)lds32(hdr);
-    for (int j = cw; j < n_out; j += NWC) {
+    // sites are dealt to the consumer warps round robin, continuing across tiles (tile sizes are not multiples of NWC)
+    for (int j = cw >= rot ? cw - rot : cw - rot + NWC; j < n_out; j += NWC) {
       const int site = (int)lds32(hdr + 16 + 4 * j);
       const uint2 sl = lds64(hdr + 16 + 4 * TC::TS + 8 * j);
       const unsigned have = (lds32(hdr + 16 + 12 * TC::TS + (j & ~3)) >> (8 * (j & 3))) & 0xffu;
@@ -281,6 +290,7 @@ __global__ void __launch_bounds__(TileCfg<LS>::THREADS, 1) k_hop_tile(const HopA
         }
       }
     }
+    rot = (rot + n_out) % NWC;
     __syncwarp();
     if (lane == 0) mbar_arrive(empty_u32 + 8 * stage);
     phases ^= 1u << stage;

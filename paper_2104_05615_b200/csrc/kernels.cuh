@@ -814,3 +814,4 @@ __global__ void k_build_links(const double* __restrict__ U_abi, T* __restrict__ 
 
 }  // namespace mspcg
 #include "transfer_tc.cuh"
+#include "dense5d_tma.cuh"

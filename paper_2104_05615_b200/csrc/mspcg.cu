@@ -81,6 +81,8 @@ struct mspcg_ctx {
   // device
   GeomDev gfull, gblk;
   TileSet tfull, tblk;
+  bool dense_tma = true;         // mspcg_apply_M5inv through dense5d_tma.cuh (MSPCG_M5_TMA=0: the cp.async kernel of transfer_tc.cuh)
+  int group_blocks = 0;          // Dirichlet blocks per L2-resident group of the preconditioner (0: all blocks at once); MSPCG_GROUP or mspcg_set_block_group
   bool use_tiles = true;         // MSPCG_TILE=0 in the environment selects the per-warp kernel k_hop_mma (A/B measurements)
   int *e_int_to_cb = nullptr, *o_int_to_cb = nullptr;   // FULL list index -> ABI x_cb, even / odd parity
   double* negI = nullptr;        // device [2][Ls][Ls]: minus the identity (full 2x2 operator of eq. 4, mspcg_apply_full)
@@ -90,6 +92,8 @@ struct mspcg_ctx {
   double *rho = nullptr, *pq = nullptr; float* scale = nullptr; double* sc = nullptr;  // device scalars
   double* Tm = nullptr;          // device copy of the reduced-Ls transfer matrix T_host (A10)
   double* Gdev = nullptr;        // gradient accumulator of the T training (A12)
+  float* BK2 = nullptr; uint4* fragI = nullptr;   // A/B of kernel 2 with the 5D matrix on tcgen05 (MSPCG_DENSE_TC=1): Mphi M5^-1 as [hi][s][s'], identity fragments
+  bool dense_tc_ab = false;
   float* Bm5[2] = {nullptr, nullptr};        // chirality blocks of M5^-1 and M5^-dag (fp32 [hi][s][s']) for k_dense5d_tc
   __half *Bfwd = nullptr, *Bbwd = nullptr;   // fp16 B-operand images of T and T^dag for the tcgen05 transfer kernels
   bool transfer_tc = true;       // use them when (Ls, Ls_hat) is a compiled pair and the inner storage is fp16
@@ -99,6 +103,8 @@ struct mspcg_ctx {
   void *stage_in = nullptr, *stage_out = nullptr;   // native staging for ABI-layout calls (fp64-sized)
   double *abi_in = nullptr, *abi_out = nullptr;     // device ABI buffers for the *_host calls
 };
+
+cudaError_t dense5d_tma(mspcg_ctx* c, const void* in, void* out, const float* Mimg, long n_sites, int Ls, cudaStream_t st);
 
 namespace {
 
@@ -188,6 +194,7 @@ void carve(mspcg_ctx* c, Arena& a) {
   c->negI = a.take<double>((size_t)2 * c->Ls * c->Ls);
   carve_mats(a, c->md, c->Ls); carve_mats(a, c->mf32, c->Ls); carve_frags(a, c->mfr);
   for (int d = 0; d < 2; d++) c->Bm5[d] = a.take<float>((size_t)2 * c->Ls * c->Ls);
+  c->BK2 = a.take<float>((size_t)2 * c->Ls * c->Ls); c->fragI = a.take<uint4>(64);
   if (c->Ls_hat) { carve_mats(a, c->md_hat, c->Ls_hat); carve_mats(a, c->mf32_hat, c->Ls_hat); carve_frags(a, c->mfr_hat); }
   c->rho = a.take<double>((size_t)(KMAX + 1) * L.nblk); c->pq = a.take<double>((size_t)KMAX * L.nblk);
   c->scale = a.take<float>(L.nblk); c->sc = a.take<double>(16);
@@ -248,12 +255,12 @@ cudaError_t launch_hop(mspcg_ctx* c, const HopArgs<T>& a, int nblk, cudaStream_t
   if constexpr (std::is_same<T, __half>::value) {   // fp16 storage: tensor-core kernels (hop_tile.cuh, hop_mma.cuh)
     if (a.tiles != nullptr && a.n_tiles > 0 && a.ng == 18) {   // thread-block-cooperative tile kernel
       static bool tattr = false;
-      const size_t tsm = TileCfg<LS>::SMEM;
+      const size_t tsm = TileCfg<LS, EPI>::SMEM;
       if (!tattr) { cudaFuncSetAttribute(k_hop_tile<LS, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsm); tattr = true; }
       HopArgs<__half> ab = a; ab.nblk = nblk;
       const long total = (long)nblk * a.n_tiles;
       const unsigned grid = (unsigned)(total < c->num_sms ? total : c->num_sms);   // persistent: one thread block per SM
-      { TimedLaunch tl(c, kind, st); k_hop_tile<LS, EPI><<<grid, TileCfg<LS>::THREADS, tsm, st>>>(ab); }
+      { TimedLaunch tl(c, kind, st); k_hop_tile<LS, EPI><<<grid, TileCfg<LS, EPI>::THREADS, tsm, st>>>(ab); }
       c->launches++;
       c->timing = was_timing;
       return cudaPeekAtLastError();
@@ -356,6 +363,15 @@ cudaError_t apply_normal(mspcg_ctx* c, const OpView<T>& v, MphiArgs<T> mp, const
   a.in = v.t1; a.in_stride = v.nE0; a.n_in_limit = v.nE0; a.out = v.tO; a.out_stride = v.nO; a.n_out = v.nO;
   a.nbr = v.nbrO; a.links = v.linksO; a.flip = v.flipO; a.link_stride = v.nO; a.mat1 = m.K2; a.frag1 = mf.K2; a.sg = (C)1;
   a.tiles = v.tO_lim; a.n_tiles = v.ntO_lim;
+  if (sizeof(T) == 2 && c->dense_tc_ab && !v.hat && a.tiles != nullptr && (LS == 8 || LS == 12 || LS == 16)) {
+    // A/B (MSPCG_DENSE_TC=1): kernel 2 with its Ls x Ls matrix on tcgen05 instead of on register fragments inside the
+    // hop -- the hop kernel runs with the identity matrix into the (larger) buffer w, then k_dense5d_tma applies Mphi M5^-1: one more
+    // pass over the stage vector.  Timed as one kernel-2 launch.
+    TimedLaunch tl(c, KIND_HOP_PLAIN, st);
+    HopArgs<T> h = a; h.out = v.w; h.frag1 = c->fragI;
+    if ((e = launch_hop<T, LS, EPI_PLAIN>(c, h, v.nblk, st, false)) != cudaSuccess) return e;
+    if ((e = dense5d_tma(c, v.w, v.tO, c->BK2, (long)v.nblk * v.nO, LS, st)) != cudaSuccess) return e;
+  } else
   if ((e = launch_hop<T, LS, EPI_PLAIN>(c, a, v.nblk, st)) != cudaSuccess) return e;
   // K3: on the interior sites (d = 0) y = p - M5^-1 D^w tO, w = M5^-dag y; on the halo sites of a Dirichlet block p = 0 and y is
   // not needed, so w = -(M5^-dag M5^-1) D^w tO is one contraction with the product matrix (a plain-epilogue launch on the site
@@ -437,53 +453,68 @@ template <> bool launch_transfer_tc<__half>(mspcg_ctx*, bool, const TransferArgs
 // LS is the fifth-dimension extent of the inner iteration: Ls, or Ls_hat when `reduced` (then the right-hand side is
 // T r, the operator is built from the Ls_hat matrices, and z = T^dag x + mu r; eq. 19-21).
 template <typename TIO, typename T, int LS>
-cudaError_t precond_impl(mspcg_ctx* c, const TIO* r_in, TIO* z_out, int k, bool reduced, cudaStream_t st) {
+cudaError_t precond_impl(mspcg_ctx* c, const TIO* r_in_all, TIO* z_out_all, int k, bool reduced, cudaStream_t st) {
   typedef typename std::conditional<sizeof(T) == 8, double, float>::type TX;
   const Geometry& g = c->lat.blk;
-  const int nblk = g.nblk;
-  OpView<T> v = make_view<T>(c, c->blkI, g, c->gblk, LS, reduced);
+  const int nblk = g.nblk;                 // also the stride of the per-block scalar arrays rho[it][nblk], pq[it][nblk]
+  const OpView<T> vall = make_view<T>(c, c->blkI, g, c->gblk, LS, reduced);
   c->cur_geom = 1;
   cudaError_t e;
   if ((e = cudaMemsetAsync(c->rho, 0, sizeof(double) * (size_t)(KMAX + 1) * nblk, st)) != cudaSuccess) return e;
   if ((e = cudaMemsetAsync(c->pq, 0, sizeof(double) * (size_t)KMAX * nblk, st)) != cudaSuccess) return e;
-  const float* scale = nullptr;
-  if (sizeof(T) == 2) {   // fp16 storage: rescale every block's right-hand side to max-abs 1 (R14)
-    if ((e = cudaMemsetAsync(c->scale, 0, sizeof(float) * nblk, st)) != cudaSuccess) return e;
-    { TimedLaunch tl(c, KIND_BLAS, st); k_maxabs<TIO><<<grid_sites(g.nE0, c->Ls, nblk), 128, 0, st>>>(r_in, g.nE0, c->Ls, c->scale); }
-    c->launches++;
-    scale = c->scale;
-  }
+  if (sizeof(T) == 2) { if ((e = cudaMemsetAsync(c->scale, 0, sizeof(float) * nblk, st)) != cudaSuccess) return e; }
+  // Block-resident inner CG ("L2-cache-bandwidth bound for GPUs with large cache"): the blocks are
+  // independent (R13), so all k inner iterations are run for a GROUP of G blocks before the next group is touched.  The group's
+  // vectors r, p, q, x and the stage vectors of eq. 16 live in the same G-block buffers for every group; with G chosen so that they
+  // fit in the 126 MB L2, HBM sees r in, z out and the group's links once per iteration.  G = 0: all blocks in one group.
+  const int G = (c->group_blocks > 0 && c->group_blocks < nblk) ? c->group_blocks : nblk;
+  const size_t io_blk = (size_t)g.nE0 * c->Ls * 24;       // reals of one block's part of an I/O vector (full Ls)
   T *r = (T*)c->in_r, *p = (T*)c->in_p, *q = (T*)c->in_q; TX* x = (TX*)c->in_x;
-  { TimedLaunch tl(c, KIND_BLAS, st);
-    bool done = false;
-    if (reduced && sizeof(T) == 2 && c->transfer_tc) {
-      TransferArgs ta; memset(&ta, 0, sizeof(ta));
-      ta.in = r_in; ta.out = r; ta.Bimg = c->Bfwd; ta.n_sites = g.nE0; ta.scale = scale; ta.rho0 = c->rho;
-      done = launch_transfer_tc<TIO>(c, true, ta, c->Ls, LS, nblk, st);
+  for (int g0 = 0; g0 < nblk; g0 += G) {
+    const int gn = g0 + G <= nblk ? G : nblk - g0;
+    const TIO* r_in = r_in_all + (size_t)g0 * io_blk;
+    TIO* z_out = z_out_all + (size_t)g0 * io_blk;
+    double *rho = c->rho + g0, *pq = c->pq + g0;
+    OpView<T> v = vall; v.nblk = gn;
+    v.linksE = vall.linksE + (size_t)g0 * vall.nE * 8 * vall.ng; v.linksO = vall.linksO + (size_t)g0 * vall.nO * 8 * vall.ng;
+    v.flipE = vall.flipE + (size_t)g0 * vall.nE; v.flipO = vall.flipO + (size_t)g0 * vall.nO;
+    const float* scale = nullptr;
+    if (sizeof(T) == 2) {   // fp16 storage: rescale every block's right-hand side to max-abs 1 (R14)
+      { TimedLaunch tl(c, KIND_BLAS, st); k_maxabs<TIO><<<grid_sites(g.nE0, c->Ls, gn), 128, 0, st>>>(r_in, g.nE0, c->Ls, c->scale + g0); }
+      c->launches++;
+      scale = c->scale + g0;
     }
-    if (done) {}
-    else if (reduced) k_reduce_begin<TIO, T><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(r_in, r, g.nE0, c->Ls, LS, c->Tm, scale, c->rho);
-    else k_pre_begin<TIO, T><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(r_in, r, g.nE0, LS, scale, c->rho); }
-  c->launches++;
-  for (int it = 0; it < k; it++) {
-    MphiArgs<T> mp; memset(&mp, 0, sizeof(mp));
-    mp.in = r; mp.p = p; mp.mode = 2; mp.it = it; mp.nblk = nblk; mp.rho = c->rho; mp.pq = c->pq;
-    if ((e = apply_normal<T, LS>(c, v, mp, p, q, c->pq + (size_t)it * nblk, st)) != cudaSuccess) return e;
-    { TimedLaunch tl(c, KIND_BLAS, st);
-      k_inner_update<T, TX, TIO><<<grid_sites(g.nE0, LS, nblk), 128, 0, st>>>(p, q, r, x, z_out, g.nE0, LS, it, nblk, (it == k - 1 && !reduced) ? 1 : 0,
-                                                                            c->rho, c->pq, scale); }
-    c->launches++;
-  }
-  if (reduced) {
     { TimedLaunch tl(c, KIND_BLAS, st);
       bool done = false;
-      if (sizeof(T) == 2 && c->transfer_tc) {
+      if (reduced && sizeof(T) == 2 && c->transfer_tc) {
         TransferArgs ta; memset(&ta, 0, sizeof(ta));
-        ta.in = x; ta.rin = r_in; ta.out = z_out; ta.Bimg = c->Bbwd; ta.n_sites = g.nE0; ta.scale = scale; ta.mu = c->mu_shift;
-        done = launch_transfer_tc<TIO>(c, false, ta, c->Ls, LS, nblk, st);
+        ta.in = r_in; ta.out = r; ta.Bimg = c->Bfwd; ta.n_sites = g.nE0; ta.scale = scale; ta.rho0 = rho;
+        done = launch_transfer_tc<TIO>(c, true, ta, c->Ls, LS, gn, st);
       }
-      if (!done) k_reduce_end<TX, TIO><<<grid_sites(g.nE0, c->Ls, nblk), 128, 0, st>>>(x, r_in, z_out, g.nE0, c->Ls, LS, c->Tm, scale, c->mu_shift); }
+      if (done) {}
+      else if (reduced) k_reduce_begin<TIO, T><<<grid_sites(g.nE0, LS, gn), 128, 0, st>>>(r_in, r, g.nE0, c->Ls, LS, c->Tm, scale, rho);
+      else k_pre_begin<TIO, T><<<grid_sites(g.nE0, LS, gn), 128, 0, st>>>(r_in, r, g.nE0, LS, scale, rho); }
     c->launches++;
+    for (int it = 0; it < k; it++) {
+      MphiArgs<T> mp; memset(&mp, 0, sizeof(mp));
+      mp.in = r; mp.p = p; mp.mode = 2; mp.it = it; mp.nblk = nblk; mp.rho = rho; mp.pq = pq;
+      if ((e = apply_normal<T, LS>(c, v, mp, p, q, pq + (size_t)it * nblk, st)) != cudaSuccess) return e;
+      { TimedLaunch tl(c, KIND_BLAS, st);
+        k_inner_update<T, TX, TIO><<<grid_sites(g.nE0, LS, gn), 128, 0, st>>>(p, q, r, x, z_out, g.nE0, LS, it, nblk, (it == k - 1 && !reduced) ? 1 : 0,
+                                                                              rho, pq, scale); }
+      c->launches++;
+    }
+    if (reduced) {
+      { TimedLaunch tl(c, KIND_BLAS, st);
+        bool done = false;
+        if (sizeof(T) == 2 && c->transfer_tc) {
+          TransferArgs ta; memset(&ta, 0, sizeof(ta));
+          ta.in = x; ta.rin = r_in; ta.out = z_out; ta.Bimg = c->Bbwd; ta.n_sites = g.nE0; ta.scale = scale; ta.mu = c->mu_shift;
+          done = launch_transfer_tc<TIO>(c, false, ta, c->Ls, LS, gn, st);
+        }
+        if (!done) k_reduce_end<TX, TIO><<<grid_sites(g.nE0, c->Ls, gn), 128, 0, st>>>(x, r_in, z_out, g.nE0, c->Ls, LS, c->Tm, scale, c->mu_shift); }
+      c->launches++;
+    }
   }
   return cudaPeekAtLastError();
 }
@@ -601,6 +632,16 @@ int upload_m5_images(mspcg_ctx* ctx, cudaStream_t st) {
       m[((size_t)hi * Ls + s) * Ls + sp] = (float)(((hi ^ d) == 0) ? ctx->hm.Ainv.at(s, sp) : ctx->hm.Ainv.at(sp, s));
     CUDA_OK(ctx, cudaMemcpyAsync(ctx->Bm5[d], m.data(), m.size() * sizeof(float), cudaMemcpyHostToDevice, st));
     CUDA_OK(ctx, cudaStreamSynchronize(st));
+  }
+  {  // kernel 2's matrix Mphi M5^-1 in the same form (hm.K2 is stored transposed per chirality: [ch][s'][s]) and identity fragments
+    std::vector<float> m((size_t)2 * Ls * Ls);
+    for (int hi = 0; hi < 2; hi++) for (int s = 0; s < Ls; s++) for (int sp = 0; sp < Ls; sp++)
+      m[((size_t)hi * Ls + s) * Ls + sp] = (float)ctx->hm.K2[((size_t)hi * Ls + sp) * Ls + s];
+    CUDA_OK(ctx, cudaMemcpyAsync(ctx->BK2, m.data(), m.size() * sizeof(float), cudaMemcpyHostToDevice, st));
+    CUDA_OK(ctx, cudaStreamSynchronize(st));
+    HostMats id; for (std::vector<double>* v : {&id.K2, &id.K3a, &id.K3b, &id.K4, &id.K5, &id.K3h}) { v->assign((size_t)2 * Ls * Ls, 0.0); for (int ch = 0; ch < 2; ch++) for (int i = 0; i < Ls; i++) (*v)[((size_t)ch * Ls + i) * Ls + i] = 1.0; }
+    MatFrag mf; mf.K2 = mf.K3a = mf.K3b = mf.K4 = mf.K5 = mf.K3h = ctx->fragI;
+    CUDA_OK(ctx, upload_frags(mf, id, Ls, st));
   }
   return MSPCG_OK;
 }
@@ -897,6 +938,7 @@ int train_eval_impl(mspcg_ctx* c, const double* v_abi, int nvec, int k, double* 
   const int Ls = c->Ls, Lh = c->Ls_hat;
   const long Vh = c->lat.V4 / 2, nreal = v5h(c, Ls) * 24;
   const size_t nG = (size_t)16 * Lh * Ls * 2;
+  struct NoGroups { mspcg_ctx* c; int g; NoGroups(mspcg_ctx* c_) : c(c_), g(c_->group_blocks) { c->group_blocks = 0; } ~NoGroups() { c->group_blocks = g; } } no_groups(c);   // in_x must hold every block
   double *V = (double*)c->stage_in, *W = (double*)c->stage_out, *E = c->v_t64, *Gv = c->v_rhi;
   const int spb = 32;
   const unsigned oblocks = (unsigned)((Vh + spb - 1) / spb);
@@ -957,6 +999,48 @@ double quartic_argmin(const double eta[5], const double val[5]) {
   return bx * sc;
 }
 
+// out = (Ls x Ls chirality blocks Mimg) in on fp16 NATIVE vectors of n_sites site columns: tensor-map TMA + tcgen05 (dense5d_tma.cuh).
+// cudaErrorNotSupported: Ls not compiled or the driver entry point is missing.
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                    const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static PFN_encodeTiled encode_tiled_fn() {
+  static PFN_encodeTiled fn = nullptr; static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* p = nullptr; cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess) fn = (PFN_encodeTiled)p;
+  }
+  return fn;
+}
+// 4D map of an fp16 NATIVE vector with the dimension order (16-byte chunk, site, s, colour): see dense5d_tma.cuh
+static bool native_f16_map(CUtensorMap* m, const void* base, long n_sites, int Ls) {
+  PFN_encodeTiled enc = encode_tiled_fn();
+  if (!enc) return false;
+  const cuuint64_t dims[4] = {8, (cuuint64_t)n_sites, (cuuint64_t)Ls, 3};
+  const cuuint64_t strides[3] = {(cuuint64_t)Ls * 48, 48, 16};
+  const cuuint32_t box[4] = {8, 128, (cuuint32_t)Ls, 3}, estr[4] = {1, 1, 1, 1};
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 4, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+cudaError_t dense5d_tma(mspcg_ctx* c, const void* in, void* out, const float* Mimg, long n_sites, int Ls, cudaStream_t st) {
+  CUtensorMap mi, mo;
+  if (!native_f16_map(&mi, in, n_sites, Ls) || !native_f16_map(&mo, out, n_sites, Ls)) return cudaErrorNotSupported;
+  Dense5dTmaArgs a; a.M = Mimg; a.n_sites = n_sites;
+  const long n_tiles = (n_sites + 127) / 128;
+  const unsigned grid = (unsigned)(n_tiles < c->num_sms ? n_tiles : c->num_sms);
+#define DT(LSV)                                                                                                            \
+  if (Ls == LSV) {                                                                                                         \
+    static bool attr = false;                                                                                              \
+    if (!attr) { cudaFuncSetAttribute(k_dense5d_tma<LSV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Dense5dTmaCfg<LSV>::SMEM); attr = true; } \
+    k_dense5d_tma<LSV><<<grid, Dense5dTmaCfg<LSV>::THREADS, Dense5dTmaCfg<LSV>::SMEM, st>>>(mi, mo, a);                  \
+    c->launches++;                                                                                                         \
+    return cudaPeekAtLastError();                                                                                          \
+  }
+  DT(8) DT(12) DT(16)
+#undef DT
+  return cudaErrorNotSupported;
+}
+
 // ================================================================================================== C ABI
 extern "C" {
 
@@ -972,7 +1056,10 @@ int mspcg_create(mspcg_ctx** out, int Lx, int Ly, int Lz, int Lt, int Ls, double
   if (!build_lattice(ctx->lat, L, B)) { delete ctx; return MSPCG_EINVAL; }
   ctx->Ls = Ls; ctx->b = b; ctx->c = c; ctx->M5 = M5; ctx->mf = mf;
   { const char* e = getenv("MSPCG_TRANSFER_TC"); if (e && e[0] == '0') ctx->transfer_tc = false; }
-  { const char* e = getenv("MSPCG_TILE"); if (e && e[0] == '0') ctx->use_tiles = false; }             // A/B switch: per-warp hop kernel   // debugging switch: generic transfer kernels
+  { const char* e = getenv("MSPCG_TILE"); if (e && e[0] == '0') ctx->use_tiles = false; }
+  { const char* e = getenv("MSPCG_GROUP"); if (e) ctx->group_blocks = atoi(e); }
+  { const char* e = getenv("MSPCG_M5_TMA"); if (e && e[0] == '0') ctx->dense_tma = false; }
+  { const char* e = getenv("MSPCG_DENSE_TC"); if (e && e[0] == '1') ctx->dense_tc_ab = true; }             // A/B switch: per-warp hop kernel   // debugging switch: generic transfer kernels
   ctx->alpha = b * (4.0 - M5) + 1.0; ctx->beta = c * (4.0 - M5) - 1.0;
   if (!build_host_mats(ctx->hm, Ls, b, c, M5, mf)) { delete ctx; return MSPCG_EINVAL; }
   *out = ctx;
@@ -1099,6 +1186,11 @@ int mspcg_apply_M5inv(mspcg_ctx* ctx, const void* in_dev, void* out_dev, int dag
   int rc = check_ready(ctx, false); if (rc) return rc;
   if (!in_dev || !out_dev || in_dev == out_dev) return fail(ctx, MSPCG_EINVAL, "bad pointer or aliasing");
   cudaStream_t st = (cudaStream_t)stream;
+  if (ctx->dense_tma) {   // tensor-map TMA + tcgen05 kernel (dense5d_tma.cuh); MSPCG_M5_TMA=0 selects the cp.async kernel below
+    cudaError_t e = dense5d_tma(ctx, in_dev, out_dev, ctx->Bm5[dagger ? 1 : 0], (long)(v5h(ctx, ctx->Ls) / ctx->Ls), ctx->Ls, st);
+    if (e == cudaSuccess) return MSPCG_OK;
+    if (e != cudaErrorNotSupported) return fail(ctx, MSPCG_ECUDA, "k_dense5d_tma: %s", cudaGetErrorString(e));
+  }
   Dense5dTcArgs a;
   a.in = reinterpret_cast<const uint4*>(in_dev); a.out = reinterpret_cast<uint4*>(out_dev);
   a.M = ctx->Bm5[dagger ? 1 : 0]; a.n_sites = (long)(v5h(ctx, ctx->Ls) / ctx->Ls);
@@ -1314,6 +1406,12 @@ int mspcg_train_T(mspcg_ctx* ctx, const double* v_dev, int nvec, int n_inner, in
   if ((rc = mspcg_train_eval(ctx, v_dev, nvec, n_inner, &val, nullptr, stream))) return rc;
   if (chi2_history_host) chi2_history_host[n_steps] = val;
   memcpy(T_host_out, T.data(), n * sizeof(double));
+  return MSPCG_OK;
+}
+
+int mspcg_set_block_group(mspcg_ctx* ctx, int blocks_per_group) {
+  if (!ctx || blocks_per_group < 0) return MSPCG_EINVAL;
+  ctx->group_blocks = blocks_per_group;
   return MSPCG_OK;
 }
 

@@ -204,6 +204,37 @@ def test_solve_mixed_precision_reliable_updates():
     assert s["converged"] == 1 and s["iters"] <= 1
 
 
+@pytest.mark.parametrize("inner,tol", [(F64, 1e-12), (F16, 2e-3)])
+def test_block_groups_give_the_same_preconditioner(inner, tol):
+    """the L2-resident schedule (all inner iterations for G blocks at a time, same buffers for every group) changes
+    the order of work only: blocks are independent (R13).  16 blocks in groups of 3 (ragged last group) and of 1, against the
+    oracle and against the ungrouped result; the reduced-Ls path too."""
+    from oracle import Oracle, reduced_ls
+    dims, Ls, block, k = (4, 8, 4, 8), 8, (2, 4, 2, 4), 4
+    import torch
+    U = synth.gauge_natural_to_abi(synth.random_su3_links(dims, 0.3, 5), dims)
+    ora = OracleC(dims, Ls, MOB["b"], MOB["c"], MOB["M5"], 0.02, block)
+    ora.load_gauge(U, -1)
+    T = reduced_ls.initial_T(Ls, 4)
+    g = Mspcg(dims, Ls, MOB["b"], MOB["c"], MOB["M5"], 0.02, block)
+    g.set_reduced_ls(4, reduced_ls.T_to_abi(T), 0.5)
+    g.configure(F64 if inner == F64 else F32, inner, 18)
+    g.load_gauge(U, -1)
+    r = synth.gaussian_spinor_abi(dims, Ls, 11)
+    d = dev(torch, r)
+    ref = ora.apply_precond(r, k)
+    z0 = g.apply_precond(d, k, F64).cpu().numpy()
+    zr0 = g.apply_precond(d, k, F64, use_reduced=1).cpu().numpy()
+    assert rel(z0, ref) <= (1e-9 if inner == F64 else 2e-2)
+    for G in (3, 1):
+        g.set_block_group(G)
+        assert rel(g.apply_precond(d, k, F64).cpu().numpy(), z0) <= tol
+        assert rel(g.apply_precond(d, k, F64, use_reduced=1).cpu().numpy(), zr0) <= tol
+    x, st = g.solve(d, tol=1e-10, use_precond=True, n_inner=k, sloppy_prec=F64 if inner == F64 else F32)
+    assert st["rc"] == 0 and st["true_res"] <= 1e-10
+    g.close()
+
+
 def test_error_codes():
     import torch
     g = Mspcg((4, 4, 4, 4), 8, 1.5, 0.5, 1.8, 0.01, (2, 2, 2, 2))
