@@ -20,6 +20,7 @@
 // stays inside one Dirichlet block for many tiles (one atomic per warp and Dirichlet block for the fused <p, A p>).
 // Links carry the antiperiodic sign already (18 reals; the 12-real format keeps the per-warp kernel).
 #pragma once
+#include <type_traits>
 #include "tile_tables.hpp"
 
 namespace mspcg {
@@ -33,8 +34,9 @@ namespace mspcg {
 template <int LS, int EPI = 0> struct TileCfg {
   enum {
     TS = TILE_TS, NIN = TILE_NIN, NSTAGE = 2,
-    NWC = (EPI == 0 ? MSPCG_TILE_NWC_PLAIN : 16),   // consumer warps (the plain epilogue needs fewer registers: more warps fit)
-    NWP = (EPI == 0 ? MSPCG_TILE_NWP_PLAIN : 4),    // producer warps
+    NWC = MSPCG_TILE_NWC_PLAIN,                     // consumer warps
+    PAIR = (MSPCG_TILE_NWC_PLAIN <= 12),            // two sites per warp in one instruction stream (needs 128 registers: at most 12 + 4 warps)
+    NWP = MSPCG_TILE_NWP_PLAIN,                     // producer warps
     COL = LS * 48,                       // bytes of one site column
     LINKREC = 8 * 18 * 2,                // bytes of the eight links of one output site
     OFF_ZERO = NIN * COL,                // one column of zeros: the slot of every absent neighbour (and of the pad lanes' link words)
@@ -87,6 +89,27 @@ __device__ __forceinline__ void hop_mu_full(float (&S)[MmaCfg<LS>::NMT][4], cons
     mma16816_4(S0[2], S0[3], S1[2], S1[3], g0, g1, c0, c1, bf, bb);
   }
 }
+// The same with the lower half spinor taken from the upper one: h' = c G^dag h, and G^dag = i sigma_k is a permutation of the two spin rows
+// times a phase, so  lower += W h' = (c phase W) (rows of h permuted, one row negated for mu = y, z):  the phase and the sign c go into a
+// second B fragment of the link (vf, vb: one byte permute each per direction and SITE), the row permutation is a choice of registers.
+//   mu = x: h' = c i (h1, h0)    mu = y: h' = c (h1, -h0)    mu = z: h' = c i (h0, -h1)    mu = t: h' = c (h0, h1)
+// 32 packed fp16 FMAs and 16 permutes per site column less than hop_mu_full, and h' is exact given h.
+template <int MU, int LS>
+__device__ __forceinline__ void hop_mu_perm(float (&S)[MmaCfg<LS>::NMT][4], const uint4 (&F)[MmaCfg<LS>::NSEG], const uint4 (&B)[MmaCfg<LS>::NSEG],
+                                            uint32_t bf, uint32_t bb, uint32_t vf, uint32_t vb, const HsConst& k) {
+#pragma unroll
+  for (int seg = 0; seg < MmaCfg<LS>::NSEG; seg++) {
+    uint32_t f0, f1, b0, b1;
+    project_hs<MU, true>(F[seg], k, f0, f1);
+    project_hs<MU, false>(B[seg], k, b0, b1);
+    float (&S0)[4] = S[2 * seg], (&S1)[4] = S[2 * seg + 1];
+    mma16816_4(S0[0], S0[1], S1[0], S1[1], f0, f1, b0, b1, bf, bb);
+    if (MU == 0)      mma16816_4(S0[2], S0[3], S1[2], S1[3], f1, f0, b1, b0, vf, vb);
+    else if (MU == 1) mma16816_4(S0[2], S0[3], S1[2], S1[3], f1, f0 ^ 0x80008000u, b1, b0 ^ 0x80008000u, vf, vb);
+    else if (MU == 2) mma16816_4(S0[2], S0[3], S1[2], S1[3], f0, f1 ^ 0x80008000u, b0, b1 ^ 0x80008000u, vf, vb);
+    else              mma16816_4(S0[2], S0[3], S1[2], S1[3], f0, f1, b0, b1, vf, vb);
+  }
+}
 
 template <int LS, int EPI>
 __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const HopArgs<__half> a) {
@@ -119,6 +142,9 @@ __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const
     // Warp w fetches the input slots [w NIN/NWP, (w+1) NIN/NWP) (a lane issues a copy for each of its slots where a run starts)
     // and the link records of the output sites [w TS/NWP, (w+1) TS/NWP); warp 0 also fetches the tile header.  Every producer warp posts
     // the bytes of its own copies on the stage's `full` barrier (arrival count NWP) before it issues them.
+#ifdef MSPCG_TILE_PURE
+    return;
+#endif
     int stage = 0, blk = blk0, ti = ti0;
     uint32_t phases = 0xffffffffu;   // bit s: parity to wait for on empty[s]; a fresh barrier passes a wait on the phase before its first one
     constexpr int SPW = TC::NIN / TC::NWP / 32;        // input slots per lane
@@ -167,7 +193,15 @@ __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const
   const bool st0 = t < 3 && g < Cfg::N0, st1 = Cfg::NSEG == 2 && t < 3 && g < Cfg::N1;
   const bool lk_mine = t < 3 && g < 6;
   const uint32_t lk_off = (uint32_t)(lk_mine ? ((g >> 1) * 3 + t) : 0);   // this lane's word inside an 18-real link
-  const uint32_t bsel = (g & 1) ? 0x1032u : 0x7610u;
+  // B fragments by one byte permute of (raw, N), raw = (Wr, Wi) the lane's complex link entry, N = -raw.  Lanes with even g hold the real
+  // output column (Xr, -Xi) of a matrix X, odd g the imaginary one (Xi, Xr):
+  //   X = W: (Wr, -Wi) | (Wi, Wr)     X = -W: (-Wr, Wi) | (-Wi, -Wr)     X = iW: (-Wi, -Wr) | (Wr, -Wi)     X = -iW: (Wi, Wr) | (-Wr, Wi)
+  const bool odd = (g & 1) != 0;
+  const uint32_t bsel = odd ? 0x1032u : 0x7610u;
+  const uint32_t sel_p = bsel, sel_m = odd ? 0x5476u : 0x3254u, sel_ip = odd ? 0x7610u : 0x5476u, sel_im = odd ? 0x3254u : 0x1032u;
+  const bool sgp = a.sg > 0;                   // c = -sg forward, +sg backward
+  const uint32_t vsel_f13 = sgp ? sel_m : sel_p, vsel_b13 = sgp ? sel_p : sel_m;      // mu = y, t: c W
+  const uint32_t vsel_f02 = sgp ? sel_im : sel_ip, vsel_b02 = sgp ? sel_ip : sel_im;  // mu = x, z: c i W
   const int lk_step = lk_mine ? 9 : 0;
 
   float part = 0.f;
@@ -201,56 +235,68 @@ __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const
     if (EPI == EPI_XPAY && a.dot_out) dot4 = reinterpret_cast<const uint4*>(a.dotv) + (long)blk * a.dotv_stride * (LS * 3);
 
     const uint32_t sb = sm_u32 + stage * TC::STAGE;
+#ifndef MSPCG_TILE_PURE
     mbar_wait(full_u32 + 8 * stage, (phases >> stage) & 1u);
+#endif
     const uint32_t hdr = sb + TC::OFF_HDR;
     const uint4* stg4 = reinterpret_cast<const uint4*>(smraw + stage * TC::STAGE);
     const uint32_t* lk32 = reinterpret_cast<const uint32_t*>(smraw + stage * TC::STAGE + TC::OFF_LINK);
     const uint32_t* zero32 = reinterpret_cast<const uint32_t*>(smraw + stage * TC::STAGE + TC::OFF_ZERO);
+#ifdef MSPCG_TILE_PURE
+    const int n_out = 32;
+#else
     const int n_out = (int)lds32(hdr);
-    // sites are dealt to the consumer warps round robin, continuing across tiles (tile sizes are not multiples of NWC)
-    for (int j = cw >= rot ? cw - rot : cw - rot + NWC; j < n_out; j += NWC) {
-      const int site = (int)lds32(hdr + 16 + 4 * j);
-      const uint2 sl = lds64(hdr + 16 + 4 * TC::TS + 8 * j);
-      const unsigned have = (lds32(hdr + 16 + 12 * TC::TS + (j & ~3)) >> (8 * (j & 3))) & 0xffu;
-      uint4 dv[NSEG], av[NSEG];
+#endif
+    // One output site in three pieces, so that two sites can be worked on in the same straight-line code (TC::PAIR, below).  Measured at C2
+    // (DESIGN.md section 4): 12 consumer warps x 2 sites per warp run exactly as fast as 16 x 1 (K2/K4 0.0727 vs 0.0723 ms), as do 20 and 24
+    // warps at 80 / 72 registers -- the kernel is bound by its per-site instruction stream on the ALU / FMA pipes, not by latency.
+    struct SiteCtx { int site; uint2 sl; unsigned have; uint4 av[NSEG], dv[NSEG]; float S[NMT][4]; const uint32_t* lkb; };
+    auto begin = [&](SiteCtx& x, const int j) {
+#ifdef MSPCG_TILE_PURE
+      x.site = (int)(((long)ti * 32 + j) % a.n_out); x.sl = make_uint2(0x03020100u + 0x04040404u * (j & 15), 0x07060504u + 0x04040404u * (j & 15)); x.have = 0xffu;
+#else
+      x.site = (int)lds32(hdr + 16 + 4 * j);
+      x.sl = lds64(hdr + 16 + 4 * TC::TS + 8 * j);
+      x.have = (lds32(hdr + 16 + 12 * TC::TS + (j & ~3)) >> (8 * (j & 3))) & 0xffu;
+#endif
       if (EPI != EPI_PLAIN) {
-        const bool ok = site < a.n_aux;
-        const uint4* p = aux4 + (long)site * (LS * 3);
-        av[0] = (ok && st0) ? __ldg(p + fo0) : make_uint4(0, 0, 0, 0);
-        if (NSEG == 2) av[NSEG - 1] = (ok && st1) ? __ldg(p + fo1) : make_uint4(0, 0, 0, 0);
+        const bool ok = x.site < a.n_aux;
+        const uint4* p = aux4 + (long)x.site * (LS * 3);
+        x.av[0] = (ok && st0) ? __ldg(p + fo0) : make_uint4(0, 0, 0, 0);
+        if (NSEG == 2) x.av[NSEG - 1] = (ok && st1) ? __ldg(p + fo1) : make_uint4(0, 0, 0, 0);
       }
       if (EPI == EPI_XPAY && dot4 != nullptr) {
-        const uint4* p = dot4 + (long)site * (LS * 3);
-        dv[0] = st0 ? __ldg(p + fo0) : make_uint4(0, 0, 0, 0);
-        if (NSEG == 2) dv[NSEG - 1] = st1 ? __ldg(p + fo1) : make_uint4(0, 0, 0, 0);
+        const uint4* p = dot4 + (long)x.site * (LS * 3);
+        x.dv[0] = st0 ? __ldg(p + fo0) : make_uint4(0, 0, 0, 0);
+        if (NSEG == 2) x.dv[NSEG - 1] = st1 ? __ldg(p + fo1) : make_uint4(0, 0, 0, 0);
       }
-      uint32_t bfr[8];
-      {  // B fragments: this lane's complex entry of each link as (Wr, -Wi) or (Wi, Wr); pad lanes read zeros
-        const uint32_t* lkb = lk_mine ? lk32 + j * (TC::LINKREC / 4) + lk_off : zero32;
+      x.lkb = lk_mine ? lk32 + j * (TC::LINKREC / 4) + lk_off : zero32;   // pad lanes read zeros
 #pragma unroll
-        for (int d = 0; d < 8; d++) {
-          const uint32_t raw = lkb[d * lk_step];
-          bfr[d] = __byte_perm(raw, raw ^ 0x80000000u, bsel);
-        }
-      }
-      float S[NMT][4];
+      for (int m = 0; m < NMT; m++) { x.S[m][0] = x.S[m][1] = x.S[m][2] = x.S[m][3] = 0.f; }
+    };
+    // direction pair MU: B fragments of the two links (this lane's complex entry as (Wr, -Wi) or (Wi, Wr), and the phase-carrying
+    // variant for the lower components), the two neighbour columns from their slots, projections and MMAs
+    auto hop_mu = [&](auto mu_tag, SiteCtx& x) {
+      constexpr int MU = decltype(mu_tag)::value;
+      uint32_t bf[2], bv[2];
 #pragma unroll
-      for (int m = 0; m < NMT; m++) { S[m][0] = S[m][1] = S[m][2] = S[m][3] = 0.f; }
-#define MSPCG_TILE_MU(MU, COND)                                                                        \
-      if (COND) {                                                                                      \
-        uint4 Ff[NSEG], Bb[NSEG];                                                                      \
-        const uint32_t w2 = (MU < 2 ? sl.x : sl.y) >> (16 * (MU & 1));                                 \
-        const uint4* pf = stg4 + (w2 & 0xffu) * (TC::COL / 16);                                        \
-        const uint4* pb = stg4 + ((w2 >> 8) & 0xffu) * (TC::COL / 16);                                 \
-        Ff[0] = pf[fo0]; Bb[0] = pb[fo0];                                                              \
-        if (NSEG == 2) { Ff[NSEG - 1] = pf[fo1]; Bb[NSEG - 1] = pb[fo1]; }                             \
-        hop_mu_full<MU, LS>(S, Ff, Bb, bfr[2 * MU], bfr[2 * MU + 1], hsk);                           \
+      for (int bw = 0; bw < 2; bw++) {
+        const uint32_t raw = x.lkb[(2 * MU + bw) * lk_step], neg = raw ^ 0x80008000u;
+        bf[bw] = __byte_perm(raw, neg, bsel);
+        bv[bw] = __byte_perm(raw, neg, (MU & 1) ? (bw ? vsel_b13 : vsel_f13) : (bw ? vsel_b02 : vsel_f02));
       }
-      MSPCG_TILE_MU(0, have & 0x03u) MSPCG_TILE_MU(1, have & 0x0cu) MSPCG_TILE_MU(2, have & 0x30u) MSPCG_TILE_MU(3, have & 0xc0u)
-#undef MSPCG_TILE_MU
-
+      uint4 Ff[NSEG], Bb[NSEG];
+      const uint32_t w2 = (MU < 2 ? x.sl.x : x.sl.y) >> (16 * (MU & 1));
+      const uint4* pf = stg4 + (w2 & 0xffu) * (TC::COL / 16);
+      const uint4* pb = stg4 + ((w2 >> 8) & 0xffu) * (TC::COL / 16);
+      Ff[0] = pf[fo0]; Bb[0] = pb[fo0];
+      if (NSEG == 2) { Ff[NSEG - 1] = pf[fo1]; Bb[NSEG - 1] = pb[fo1]; }
+      hop_mu_perm<MU, LS>(x.S, Ff, Bb, bf[0], bf[1], bv[0], bv[1], hsk);
+    };
+    auto finish = [&](SiteCtx& x) {
+      float (&S)[NMT][4] = x.S;
+      const int site = x.site;
       dense5d_mma<LS>(S, sfrag, lane);
-
       uint4 o[NSEG];
       uint4* po = out4 + (long)site * (LS * 3);
       if (EPI == EPI_PLAIN) {
@@ -259,7 +305,7 @@ __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const
         if (NSEG == 2) { if (st1) po[fo1] = o[NSEG - 1]; }
       } else {
         float V[NMT][4];
-        frag_to_float<LS>(av, V);
+        frag_to_float<LS>(x.av, V);
 #pragma unroll
         for (int m = 0; m < NMT; m++) {
 #pragma unroll
@@ -279,7 +325,7 @@ __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const
         if (NSEG == 2) { if (st1) po[fo1] = o[NSEG - 1]; }
         if (EPI == EPI_XPAY && dot4 != nullptr) {
           float P[NMT][4];
-          frag_to_float<LS>(dv, P);
+          frag_to_float<LS>(x.dv, P);
           if (st0 || st1) {
 #pragma unroll
             for (int m = 0; m < NMT; m++) {
@@ -289,10 +335,47 @@ __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const
           }
         }
       }
+    };
+    typedef std::integral_constant<int, 0> M0; typedef std::integral_constant<int, 1> M1;
+    typedef std::integral_constant<int, 2> M2; typedef std::integral_constant<int, 3> M3;
+    // sites are dealt to the consumer warps round robin, continuing across tiles (tile sizes are not multiples of NWC)
+    int j = cw >= rot ? cw - rot : cw - rot + NWC;
+#ifdef MSPCG_TILE_PURE
+    if (true) {
+#else
+    if (lds32(hdr + 8) != 0u) {
+#endif
+      // every site of the tile has all eight neighbours (flag in the tile header): no branches, two sites at a time
+      for (; TC::PAIR && j + NWC < n_out; j += 2 * NWC) {
+        SiteCtx x0, x1;
+        begin(x0, j); begin(x1, j + NWC);
+        hop_mu(M0(), x0); hop_mu(M0(), x1); hop_mu(M1(), x0); hop_mu(M1(), x1);
+        hop_mu(M2(), x0); hop_mu(M2(), x1); hop_mu(M3(), x0); hop_mu(M3(), x1);
+        finish(x0); finish(x1);
+      }
+      for (; j < n_out; j += NWC) {
+        SiteCtx x0;
+        begin(x0, j);
+        hop_mu(M0(), x0); hop_mu(M1(), x0); hop_mu(M2(), x0); hop_mu(M3(), x0);
+        finish(x0);
+      }
+    } else {
+      // halo tiles of a Dirichlet block: direction pairs with no neighbour are skipped (a single absent neighbour reads the zero column)
+      for (; j < n_out; j += NWC) {
+        SiteCtx x0;
+        begin(x0, j);
+        if (x0.have & 0x03u) hop_mu(M0(), x0);
+        if (x0.have & 0x0cu) hop_mu(M1(), x0);
+        if (x0.have & 0x30u) hop_mu(M2(), x0);
+        if (x0.have & 0xc0u) hop_mu(M3(), x0);
+        finish(x0);
+      }
     }
     rot = (rot + n_out) % NWC;
     __syncwarp();
+#ifndef MSPCG_TILE_PURE
     if (lane == 0) mbar_arrive(empty_u32 + 8 * stage);
+#endif
     phases ^= 1u << stage;
     stage = stage + 1 == TC::NSTAGE ? 0 : stage + 1;
     if (++ti == a.n_tiles) { ti = 0; blk++; }

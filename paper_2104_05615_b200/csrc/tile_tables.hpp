@@ -26,7 +26,7 @@ constexpr int TILE_TS = 32;     // output sites per tile
 constexpr int TILE_NIN = 128;   // staged input columns per tile
 
 struct TileRec {                // 1104 bytes, 16-byte aligned; the first TILE_HDR bytes are staged for the consumer warps
-  int n_out, n_in, pad0, pad1;
+  int n_out, n_in, pad0, pad1;  // pad0: 1 if every site of the tile has all eight neighbours
   int out_site[TILE_TS];        // ascending
   uint8_t slot[TILE_TS][8];
   uint8_t have[TILE_TS];
@@ -80,6 +80,8 @@ inline std::vector<TileRec> build_tiles(const std::vector<short>& coords, const 
       }
     }
     for (int j = 0; j < cur.n_out;) { int n = 1; while (j + n < cur.n_out && members[j + n] == members[j] + n) n++; cur.out_run[j] = (uint8_t)n; j += n; }
+    cur.pad0 = 1;   // flag: every site of the tile has all eight neighbours
+    for (int j = 0; j < cur.n_out; j++) if (cur.have[j] != 0xff) cur.pad0 = 0;
     tiles.push_back(cur);
     members.clear(); slot_of.clear();
   };
