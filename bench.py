@@ -292,6 +292,9 @@ def run_ours(args):
     alg = {"blk.hop_k2k4": 0.5 * (bb["hop_k2"] + bb["hop_k4"]), "blk.hop_k3": bb["hop_k3"], "blk.hop_k5": bb["hop_k5"],
            "blk.mphi": bb["mphi"], "full.hop_k2k4": 0.5 * (bf["hop_k2"] + bf["hop_k4"]), "full.hop_k3": bf["hop_k3"],
            "full.hop_k5": bf["hop_k5"], "full.mphi": bf["mphi"]}
+    if args.group and args.group < geo["nblk"]:   # a launch covers one group of blocks only
+        ngroups = -(-geo["nblk"] // args.group)
+        alg = {n: (b / ngroups if n.startswith("blk.") else b) for n, b in alg.items()}
     kern = {}
     tot_ms = sum(v["ms"] for v in tm.values())
     for name, v in tm.items():
@@ -395,22 +398,7 @@ def extras(torch, g, cfg, U, src, d_src, geo, peak, args):
     g2.load_gauge(U, -1)
     ex["DdagD_fp16"] = time_op(g2, F16, 2)
     if Ls in (8, 12, 16):
-        # the dense 5D contraction M5^-1 on its own as a tcgen05 GEMM (mspcg_apply_M5inv): four buffer pairs in rotation
-        # (one fp16 vector pair is smaller than L2), flops by the minimal count 48*Ls per 5D site and as issued (8x: delta_jj' zeros)
-        ins = [g2.pack(d_src, F16) for _ in range(4)]
-        outs = [g2.new_native(F16) for _ in range(4)]
-        cnt = [0]
-
-        def m5():
-            g2.apply_M5inv(ins[cnt[0] & 3], False, out=outs[cnt[0] & 3])
-            cnt[0] += 1
-        ms = timed(torch, m5, 4 * steps, 4 * warm) / (4 * steps)
-        n5 = ins[0].numel() * ins[0].element_size() // 48
-        e = op_entry(ms, 48.0 * Ls * n5, 2.0 * 48 * n5)
-        e["GFLOPs_issued_on_tensor_cores"] = 8 * e["GFLOPs"]
-        e["note"] = "tcgen05.mma kind::f16, fp32 accumulation in TMEM; 4 buffer pairs rotated"
-        ex["M5inv_tcgen05_fp16"] = e
-        del ins, outs
+        ex["M5inv_tcgen05_fp16"] = time_m5inv(torch, g2, d_src, Ls, steps, warm, peak)
     ex["Mpre_k%d_fp64" % k] = time_pre(g2, F64, 8, 8)
     g2.close()
     torch.cuda.empty_cache()
@@ -497,6 +485,35 @@ def run_solves(args):
         out["solves"][name] = solve_entry(st)
     out["clocks"] = sampler.stop()
     print(json.dumps(out))
+
+
+def time_m5inv(torch, g, d_src, Ls, steps, warm, peak):
+    """The dense 5D contraction M5^-1 on its own as a tcgen05 GEMM (mspcg_apply_M5inv): four buffer pairs in rotation (one fp16
+    vector pair is smaller than L2); flops by the minimal count 48*Ls per 5D site and as issued (8x: the delta_jj' zeros of the B operand)."""
+    from paper_2104_05615_b200 import F16
+    ins = [g.pack(d_src, F16) for _ in range(4)]
+    outs = [g.new_native(F16) for _ in range(4)]
+    cnt = [0]
+
+    def m5():
+        g.apply_M5inv(ins[cnt[0] & 3], False, out=outs[cnt[0] & 3])
+        cnt[0] += 1
+    ms = timed(torch, m5, 4 * steps, 4 * warm) / (4 * steps)
+    n5 = ins[0].numel() * ins[0].element_size() // 48
+    nbytes, flops = 2.0 * 48 * n5, 48.0 * Ls * n5
+    return dict(ms=ms, GFLOPs=flops / (ms * 1e-3) / 1e9, GBps_algorithmic=nbytes / (ms * 1e-3) / 1e9, hbm_frac=nbytes / (ms * 1e-3) / 1e9 / peak,
+                GFLOPs_issued_on_tensor_cores=8 * flops / (ms * 1e-3) / 1e9,
+                note="tcgen05.mma kind::f16, fp32 accumulation in TMEM, operands and results moved by tensor-map TMA; 4 buffer pairs rotated")
+
+
+def run_m5inv(args):
+    import torch
+    from paper_2104_05615_b200 import F16, Mspcg
+    cfg = synth.CONFIGS[args.workload]
+    g = Mspcg(cfg["dims"], cfg["Ls"], cfg["b"], cfg["c"], cfg["M5"], cfg["mf"], cfg["block"])
+    g.configure(F16, F16, 18)
+    d_src = torch.as_tensor(synth.gaussian_spinor_abi(cfg["dims"], cfg["Ls"], cfg["src_seed"]).reshape(-1)).cuda()
+    print(json.dumps(dict(impl="ours", mode="m5inv", workload=args.workload, M5inv_tcgen05_fp16=time_m5inv(torch, g, d_src, cfg["Ls"], max(3, args.steps), 3, peaks()[0]))))
 
 
 def oracle_sample(cfg, U, src, geo):
@@ -621,6 +638,7 @@ def main():
     ap.add_argument("--train-steps", type=int, default=100, help="line-search steps of the T training in the extras")
     ap.add_argument("--mu", type=float, default=0.85, help="shift mu of the reduced-Ls preconditioner in the extras (PAPER.md:309 eq. 20; the paper's tuned values: 0.437-0.85)")
     ap.add_argument("--cpu-solves", default="", choices=["", "C1", "C3p"], help="with --impl reference: full CG and MSPCG solves on the CPU oracle on this lattice (C3p = reduced C3: 12^3 x 24, Ls 8)")
+    ap.add_argument("--m5inv-only", action="store_true", help="time only the stand-alone M5^-1 contraction (mspcg_apply_M5inv) on the workload and print its entry")
     ap.add_argument("--group", type=int, default=0, help="Dirichlet blocks per L2-resident group of the preconditioner (mspcg_set_block_group; 0 = all at once)")
     ap.add_argument("--solves", action="store_true", help="time to solution instead of the step benchmark: CG, MSPCG (and reduced-Ls MSPCG with --reduced-solve) on --workload")
     ap.add_argument("--reduced-solve", action="store_true", help="with --solves: also train T on a sample lattice and solve with the reduced-Ls preconditioner")
@@ -632,6 +650,8 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
+    elif args.m5inv_only:
+        run_m5inv(args)
     elif args.solves:
         run_solves(args)
     else:
