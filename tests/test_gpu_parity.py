@@ -235,6 +235,32 @@ def test_block_groups_give_the_same_preconditioner(inner, tol):
     g.close()
 
 
+@pytest.mark.parametrize("inner", [F64, F16])
+def test_poisoned_neighbour_blocks_do_not_leak(inner):
+    """Stand-in for the memory checker the GPU pool refuses: every input element OUTSIDE one Dirichlet block is NaN.
+    A_s and M^-1 of that block read nothing but the block ("without communication"; the snake terms are temporaries computed
+    from the block's own sites), so its output must be finite and what it is with clean neighbours; any read past
+    the block -- a wrong neighbour index, a tile slot of another block, a run one column too long -- turns it into NaN."""
+    dims, Ls, block, k = (8, 4, 8, 8), 8, (4, 2, 4, 4), 3
+    ora, g, torch = setup(dims, Ls, 0.02, block, outer=F64 if inner == F64 else F32, inner=inner)
+    v = synth.gaussian_spinor_abi(dims, Ls, 4)
+    d = dev(torch, v)
+    for blk in (0, 5, ora.num_blocks - 1):
+        mask = torch.as_tensor(ora.apply_A_block(np.ones_like(v), blk).reshape(-1) != 0).cuda()   # the block's own sites
+        assert int(mask.sum()) == v.size // ora.num_blocks
+        poisoned = torch.where(mask, d, torch.full_like(d, float("nan")))
+        clean = torch.where(mask, d, torch.zeros_like(d))
+        if inner == F64:
+            a_p, a_c = g.apply_A_block(poisoned, blk, F64), g.apply_A_block(clean, blk, F64)
+            assert bool(torch.isfinite(a_p).all()) and bool((a_p == a_c).all())
+        z_p, z_c = g.apply_precond(poisoned, k, F64), g.apply_precond(clean, k, F64)
+        assert bool(torch.isfinite(z_p[mask]).all())
+        # equal up to the order of the atomic partial sums of the block's inner products
+        assert rel(z_p[mask].cpu().numpy(), z_c[mask].cpu().numpy()) <= (1e-12 if inner == F64 else 2e-3)
+        assert bool(torch.isnan(z_p[~mask]).any())            # the poison did reach the other blocks' own solves (the test has teeth)
+    g.close()
+
+
 def test_error_codes():
     import torch
     g = Mspcg((4, 4, 4, 4), 8, 1.5, 0.5, 1.8, 0.01, (2, 2, 2, 2))
