@@ -189,6 +189,14 @@ int mspcg_residual(mspcg_ctx* ctx, const double* b_dev, const double* x_dev, dou
  * interact, R13).  The environment variable MSPCG_GROUP sets the default of new contexts.  Errors: MSPCG_EINVAL (G < 0). */
 int mspcg_set_block_group(mspcg_ctx* ctx, int blocks_per_group);
 
+/* Host-only self check of the site tiles of the fp16 tile kernel (hop_tile.cuh; needs no GPU and no workspace): builds the tile tables of
+ * the Dirichlet-block and the full-lattice geometry and verifies them against the neighbour tables (every output site in exactly one
+ * tile, every neighbour's shared-memory slot holding that neighbour's column, absent neighbours on the zero column, copy runs consecutive
+ * and complete).  out_host[8] (HOST): [0] 0 or a failure code, [1..4] tiles per block of kernel 2, kernel 4, kernels 3/5 (interior), kernel 3
+ * (halo), [5..7] staged input columns per output site (8 without reuse) for kernel 4, for kernels 3/5, for the full lattice.
+ * Errors: MSPCG_EINVAL (null pointer, or inconsistent tables: see mspcg_last_error). */
+int mspcg_tile_check(mspcg_ctx* ctx, double out_host[8]);
+
 /* Counters for reports: kernels launched by this context since creation. */
 long mspcg_launch_count(const mspcg_ctx* ctx);
 

@@ -24,7 +24,7 @@ SYMBOLS = [
     "mspcg_unpack", "mspcg_apply_MdagM", "mspcg_apply_precond", "mspcg_apply_MdagM_host",
     "mspcg_apply_precond_host", "mspcg_apply_A_block", "mspcg_set_reduced_ls", "mspcg_solve", "mspcg_launch_count",
     "mspcg_timing", "mspcg_timing_read", "mspcg_update_T", "mspcg_train_eval", "mspcg_train_T",
-    "mspcg_prepare_source", "mspcg_reconstruct_odd", "mspcg_apply_full", "mspcg_apply_M5inv", "mspcg_residual", "mspcg_set_block_group",
+    "mspcg_prepare_source", "mspcg_reconstruct_odd", "mspcg_apply_full", "mspcg_apply_M5inv", "mspcg_residual", "mspcg_set_block_group", "mspcg_tile_check",
 ]
 
 
@@ -76,6 +76,7 @@ def load_library():
     L.mspcg_apply_full.argtypes = [vp, vp, vp, vp, vp, vp]
     L.mspcg_residual.argtypes = [vp, vp, vp, vp, i, dp, vp]
     L.mspcg_set_block_group.argtypes = [vp, i]
+    L.mspcg_tile_check.argtypes = [vp, dp]
     L.mspcg_set_reduced_ls.argtypes = [vp, i, dp, d]
     L.mspcg_solve.argtypes = [vp, vp, vp, C.POINTER(SolveParams), C.POINTER(SolveStats), vp]
     L.mspcg_launch_count.argtypes = [vp]
@@ -276,6 +277,13 @@ class Mspcg:
         self._check(self.lib.mspcg_apply_full(self.h, C.c_void_p(psi_e_abi.data_ptr()), C.c_void_p(psi_o_abi.data_ptr()),
                                               C.c_void_p(oe.data_ptr()), C.c_void_p(oo.data_ptr()), self._stream()))
         return oe, oo
+
+    def tile_check(self):
+        """Host-only consistency check of the tile tables of the fp16 tile kernel (mspcg_tile_check); raises on failure."""
+        out = np.zeros(8)
+        self._check(self.lib.mspcg_tile_check(self.h, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return dict(tiles_k2=int(out[1]), tiles_k4=int(out[2]), tiles_k3k5=int(out[3]), tiles_k3_halo=int(out[4]),
+                    inputs_per_output_k4=out[5], inputs_per_output_k3k5=out[6], inputs_per_output_full=out[7])
 
     def set_block_group(self, blocks_per_group):
         """L2-resident groups of Dirichlet blocks for the preconditioner (mspcg_set_block_group); 0 = all blocks at once."""

@@ -1409,6 +1409,25 @@ int mspcg_train_T(mspcg_ctx* ctx, const double* v_dev, int nvec, int n_inner, in
   return MSPCG_OK;
 }
 
+int mspcg_tile_check(mspcg_ctx* ctx, double out_host[8]) {
+  if (!ctx || !out_host) return MSPCG_EINVAL;
+  TileSet tb, tf;
+  build_tile_set(tb, ctx->lat.blk); build_tile_set(tf, ctx->lat.full);
+  const Geometry &g = ctx->lat.blk, &f = ctx->lat.full;
+  int bad = 0, code;
+  if ((code = check_tiles(tb.hO_lim, g.nbrO, 0, g.nO, g.nE0))) bad = 100 + code;
+  else if (!tb.hO_all.empty() && (code = check_tiles(tb.hO_all, g.nbrO, 0, g.nO, g.nE))) bad = 200 + code;
+  else if ((code = check_tiles(tb.hE_int, g.nbrE, 0, g.nE0, g.nO))) bad = 300 + code;
+  else if ((code = check_tiles(tb.hE_halo, g.nbrE, g.nE0, g.nE, g.nO))) bad = 400 + code;
+  else if ((code = check_tiles(tf.hO_lim, f.nbrO, 0, f.nO, f.nE0))) bad = 500 + code;
+  else if ((code = check_tiles(tf.hE_int, f.nbrE, 0, f.nE0, f.nO))) bad = 600 + code;
+  const std::vector<TileRec>& k4 = tb.hO_all.empty() ? tb.hO_lim : tb.hO_all;
+  out_host[0] = bad;
+  out_host[1] = (double)tb.hO_lim.size(); out_host[2] = (double)k4.size(); out_host[3] = (double)tb.hE_int.size(); out_host[4] = (double)tb.hE_halo.size();
+  out_host[5] = tiles_inputs_per_output(k4); out_host[6] = tiles_inputs_per_output(tb.hE_int); out_host[7] = tiles_inputs_per_output(tf.hE_int);
+  return bad ? fail(ctx, MSPCG_EINVAL, "tile tables inconsistent with the neighbour tables (code %d)", bad) : MSPCG_OK;
+}
+
 int mspcg_set_block_group(mspcg_ctx* ctx, int blocks_per_group) {
   if (!ctx || blocks_per_group < 0) return MSPCG_EINVAL;
   ctx->group_blocks = blocks_per_group;

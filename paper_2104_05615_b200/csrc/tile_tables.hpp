@@ -107,6 +107,47 @@ inline std::vector<TileRec> build_tiles(const std::vector<short>& coords, const 
   return tiles;
 }
 
+// Host-side check of a tiling against the neighbour table it was built from: every output site of [lo, hi) in exactly one tile, every
+// present neighbour's slot holding exactly that neighbour's column, absent ones pointing at the zero column with their presence bit clear,
+// input columns ascending and distinct, copy runs covering every slot exactly once with consecutive columns.  Returns 0 or a failure code.
+inline int check_tiles(const std::vector<TileRec>& tiles, const std::vector<int>& nbr, int lo, int hi, int in_limit) {
+  std::vector<char> seen(hi > lo ? hi - lo : 0, 0);
+  for (const TileRec& t : tiles) {
+    if (t.n_out < 1 || t.n_out > TILE_TS || t.n_in < 0 || t.n_in > TILE_NIN) return 1;
+    for (int i = 1; i < t.n_in; i++) if (t.in_col[i] <= t.in_col[i - 1]) return 2;
+    int covered = 0;
+    for (int i = 0; i < t.n_in;) {
+      const int n = t.in_run[i];
+      if (n < 1 || i + n > t.n_in) return 3;
+      for (int q = 1; q < n; q++) if (t.in_run[i + q] != 0 || t.in_col[i + q] != t.in_col[i] + q) return 4;
+      covered += n; i += n;
+    }
+    if (covered != t.n_in) return 5;
+    for (int j = 0; j < t.n_out;) {
+      const int n = t.out_run[j];
+      if (n < 1 || j + n > t.n_out) return 6;
+      for (int q = 1; q < n; q++) if (t.out_run[j + q] != 0 || t.out_site[j + q] != t.out_site[j] + q) return 7;
+      j += n;
+    }
+    bool full = true;
+    for (int j = 0; j < t.n_out; j++) {
+      const int site = t.out_site[j];
+      if (site < lo || site >= hi || seen[site - lo]) return 8;
+      seen[site - lo] = 1;
+      for (int d = 0; d < 8; d++) {
+        const int nb = nbr[(size_t)site * 8 + d];
+        const bool present = nb >= 0 && nb < in_limit;
+        if (present != (((t.have[j] >> d) & 1) != 0)) return 9;
+        if (present) { if (t.slot[j][d] >= t.n_in || t.in_col[t.slot[j][d]] != nb) return 10; }
+        else { if (t.slot[j][d] != TILE_NIN) return 11; full = false; }
+      }
+    }
+    if ((t.pad0 != 0) != full) return 12;
+  }
+  for (char c : seen) if (!c) return 13;
+  return 0;
+}
+
 // staged input columns per output site (8 without reuse): the figure of merit of a tiling
 inline double tiles_inputs_per_output(const std::vector<TileRec>& t) {
   long in = 0, out = 0;

@@ -52,6 +52,23 @@ def test_site_sets_match_golden_shell_counts(lib):
         m.close()
 
 
+@pytest.mark.parametrize("dims,block", [((16, 16, 16, 32), (8, 8, 8, 8)), ((4, 4, 4, 4), (2, 2, 2, 2)), ((2, 4, 6, 6), (2, 2, 6, 2)),
+                                        ((8, 4, 4, 6), (4, 4, 2, 6)), ((12, 12, 12, 12), (6, 6, 6, 12)), ((4, 6, 4, 4), (2, 6, 2, 2))])
+def test_tile_tables_of_the_fp16_tile_kernel(lib, dims, block):
+    """Host logic of hop_tile.cuh (tile_tables.hpp, the cell-ordered site lists of geometry.hpp): every output site of every stage list in
+    exactly one tile, every neighbour reference resolved to the shared-memory slot that holds that neighbour, absent neighbours on the
+    zero column, copy runs consecutive and complete -- on the C2 geometry, the wrap-around case L - B < 4, ragged and uncut directions.
+    Reuse: a full 4x4x2x2 cell stages 4.0 input columns per output site instead of 8."""
+    m = Mspcg(dims, 8, 1.5, 0.5, 1.8, 0.01, block)
+    st = m.tile_check()
+    g = m.geometry()
+    assert st["tiles_k3k5"] >= -(-g["nE0"] // 32) and st["tiles_k4"] >= -(-g["nO1"] // 32)
+    if dims == (16, 16, 16, 32):
+        assert st["tiles_k3k5"] == 64 and st["inputs_per_output_k3k5"] == 4.0 and st["inputs_per_output_full"] == 4.0
+        assert st["inputs_per_output_k4"] < 5.0
+    m.close()
+
+
 def test_uncut_direction_has_no_halo(lib):
     m = Mspcg((4, 4, 4, 8), 8, 1.5, 0.5, 1.8, 0.01, (4, 4, 4, 8))
     g = m.geometry()
