@@ -1,5 +1,11 @@
 """Training of the reduced-Ls transfer matrix (eq. 22) -- the library against oracle/reduced_ls.py on the same
-seeded inputs: loss, gradient (every entry) and the T sequence of the line search with momentum."""
+seeded inputs: loss, gradient (every entry) and the T sequence of the line search with momentum.
+
+What this pins and what it does not.  The loss chi2 (eq. 22) and its analytic gradient are definitions: the oracle's gradient is pinned by
+central finite differences (tests/test_oracle_reduced_ls.py), so the first two tests are parity proper.  The STEP RULE (five samples at
+eta0 (0, 1/2, 1, 3/2, 2), quartic fit, momentum dropped and eta0 quartered after a step without decrease) is a reading of the paper's two words
+"line search" and "momentum" (parity unpinned) that the oracle and the library implement alike -- the T-sequence
+test shows that the two follow the same rule to rounding, not that the rule is the paper's."""
 import numpy as np
 import pytest
 
