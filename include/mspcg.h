@@ -101,6 +101,11 @@ int mspcg_apply_MdagM_host(mspcg_ctx* ctx, const double* in_host, double* out_ho
 int mspcg_apply_precond_host(mspcg_ctx* ctx, const double* r_host, double* z_host, int io_prec, int n_inner,
                              int use_reduced);
 
+/* The same with SINGLE-precision host vectors (ABI layout psi[s][x_cb][4][3][re,im] in float, HOST, pinned for full PCIe speed): half the
+ * PCIe bytes for computations that run in fp32 or fp16 anyway.  prec / io_prec: MSPCG_F32 or MSPCG_F16 (MSPCG_EINVAL for fp64).  Synchronous. */
+int mspcg_apply_MdagM_host32(mspcg_ctx* ctx, const float* in_host, float* out_host, int prec);
+int mspcg_apply_precond_host32(mspcg_ctx* ctx, const float* r_host, float* z_host, int io_prec, int n_inner, int use_reduced);
+
 /* A_s applied to the block-`block` part of a vector (debug / parity entry: PAPER.md:224, R10): fp64, ABI layout;
  * out is zero outside the block. */
 int mspcg_apply_A_block(mspcg_ctx* ctx, const double* in_dev, double* out_dev, int block, int prec, void* stream);

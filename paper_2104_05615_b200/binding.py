@@ -24,7 +24,7 @@ SYMBOLS = [
     "mspcg_unpack", "mspcg_apply_MdagM", "mspcg_apply_precond", "mspcg_apply_MdagM_host",
     "mspcg_apply_precond_host", "mspcg_apply_A_block", "mspcg_set_reduced_ls", "mspcg_solve", "mspcg_launch_count",
     "mspcg_timing", "mspcg_timing_read", "mspcg_update_T", "mspcg_train_eval", "mspcg_train_T",
-    "mspcg_prepare_source", "mspcg_reconstruct_odd", "mspcg_apply_full", "mspcg_apply_M5inv", "mspcg_residual", "mspcg_set_block_group", "mspcg_tile_check",
+    "mspcg_prepare_source", "mspcg_reconstruct_odd", "mspcg_apply_full", "mspcg_apply_M5inv", "mspcg_residual", "mspcg_set_block_group", "mspcg_tile_check", "mspcg_apply_MdagM_host32", "mspcg_apply_precond_host32",
 ]
 
 
@@ -70,6 +70,8 @@ def load_library():
     L.mspcg_apply_precond.argtypes = [vp, vp, vp, i, i, i, i, vp]
     L.mspcg_apply_MdagM_host.argtypes = [vp, vp, vp, i]
     L.mspcg_apply_precond_host.argtypes = [vp, vp, vp, i, i, i]
+    L.mspcg_apply_MdagM_host32.argtypes = [vp, vp, vp, i]
+    L.mspcg_apply_precond_host32.argtypes = [vp, vp, vp, i, i, i]
     L.mspcg_apply_A_block.argtypes = [vp, vp, vp, i, i, vp]
     L.mspcg_prepare_source.argtypes = [vp, vp, vp, vp, vp, vp]
     L.mspcg_reconstruct_odd.argtypes = [vp, vp, vp, vp, vp]
@@ -301,6 +303,16 @@ class Mspcg:
     def apply_MdagM_host(self, v_host, out_host, prec=F64):
         self._check(self.lib.mspcg_apply_MdagM_host(self.h, C.c_void_p(v_host.data_ptr()), C.c_void_p(out_host.data_ptr()), prec))
         return out_host
+
+    def apply_MdagM_host32(self, v_host, out_host, prec=F32):
+        """float32 host tensors in the ABI layout (mspcg_apply_MdagM_host32)."""
+        self._check(self.lib.mspcg_apply_MdagM_host32(self.h, C.c_void_p(v_host.data_ptr()), C.c_void_p(out_host.data_ptr()), prec))
+        return out_host
+
+    def apply_precond_host32(self, r_host, z_host, n_inner, io_prec=F32, use_reduced=0):
+        self._check(self.lib.mspcg_apply_precond_host32(self.h, C.c_void_p(r_host.data_ptr()), C.c_void_p(z_host.data_ptr()), io_prec,
+                                                        int(n_inner), int(use_reduced)))
+        return z_host
 
     def apply_precond_host(self, r_host, z_host, n_inner, io_prec=F64, use_reduced=0):
         self._check(self.lib.mspcg_apply_precond_host(self.h, C.c_void_p(r_host.data_ptr()), C.c_void_p(z_host.data_ptr()), io_prec,

@@ -746,15 +746,15 @@ __global__ void k_axpby(double a, const T* __restrict__ x, double b, T* __restri
 }
 
 // -------------------------------------------------------------------------------- layout conversion and gauge ingest
-// ABI psi[s][x_cb][24] fp64  <->  native v[i][chunk][s][PER] (i = FULL E-list index), SURVEY 8(b).
-template <typename T, int LS>
-__global__ void k_pack(const double* __restrict__ abi, T* __restrict__ nat, const int* __restrict__ int_to_cb, long Vh, int to_native) {
+// ABI psi[s][x_cb][24] (fp64; fp32 for the *_host32 entry points)  <->  native v[i][chunk][s][PER] (i = FULL E-list index), SURVEY 8(b).
+template <typename T, int LS, typename TA>
+__global__ void k_pack(const TA* __restrict__ abi, T* __restrict__ nat, const int* __restrict__ int_to_cb, long Vh, int to_native) {
   typedef typename ST<T>::C C;
   const long i = (long)blockIdx.x * Tile<LS>::NS + threadIdx.y;
   const int s = threadIdx.x;
   if (i >= Vh) return;
   const long cb = int_to_cb[i];
-  double* a = const_cast<double*>(abi) + ((long)s * Vh + cb) * 24;
+  TA* a = const_cast<TA*>(abi) + ((long)s * Vh + cb) * 24;
   C v[24];
   if (to_native) {
 #pragma unroll
@@ -763,7 +763,7 @@ __global__ void k_pack(const double* __restrict__ abi, T* __restrict__ nat, cons
   } else {
     load24<T>(nat, i, s, LS, v);
 #pragma unroll
-    for (int k = 0; k < 24; k++) a[k] = (double)v[k];
+    for (int k = 0; k < 24; k++) a[k] = (TA)v[k];
   }
 }
 

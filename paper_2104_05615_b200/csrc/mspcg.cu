@@ -556,15 +556,19 @@ cudaError_t normal_full_any(mspcg_ctx* c, int prec, const void* p, void* q, doub
   return normal_full<__half>(c, *ob, (const __half*)p, (__half*)q, mphi_plain<__half>((const __half*)p), dot_out, st);
 }
 
-cudaError_t pack_any(mspcg_ctx* c, const double* abi, void* nat, int prec, int to_native, cudaStream_t st, int parity = 0) {
+template <typename TA>
+cudaError_t pack_any_t(mspcg_ctx* c, const TA* abi, void* nat, int prec, int to_native, cudaStream_t st, int parity) {
   const long Vh = c->lat.V4 / 2;
   const int* table = parity ? c->o_int_to_cb : c->e_int_to_cb;
 #define PK(TT) DISPATCH_LS(c->Ls, { dim3 block(LS, Tile<LS>::NS), grid((unsigned)((Vh + Tile<LS>::NS - 1) / Tile<LS>::NS)); \
-    k_pack<TT, LS><<<grid, block, 0, st>>>(abi, (TT*)nat, table, Vh, to_native); })
+    k_pack<TT, LS, TA><<<grid, block, 0, st>>>(abi, (TT*)nat, table, Vh, to_native); })
   if (prec == MSPCG_F64) PK(double) else if (prec == MSPCG_F32) PK(float) else PK(__half)
 #undef PK
   c->launches++;
   return cudaPeekAtLastError();
+}
+cudaError_t pack_any(mspcg_ctx* c, const double* abi, void* nat, int prec, int to_native, cudaStream_t st, int parity = 0) {
+  return pack_any_t<double>(c, abi, nat, prec, to_native, st, parity);
 }
 
 template <typename T>
@@ -1291,6 +1295,36 @@ int mspcg_apply_precond_host(mspcg_ctx* ctx, const double* r_host, double* z_hos
   CUDA_OK(ctx, cudaMemcpyAsync(ctx->abi_in, r_host, n, cudaMemcpyHostToDevice, 0));
   rc = mspcg_apply_precond(ctx, ctx->abi_in, ctx->abi_out, io_prec, MSPCG_LAYOUT_ABI, n_inner, use_reduced, nullptr); if (rc) return rc;
   CUDA_OK(ctx, cudaMemcpyAsync(z_host, ctx->abi_out, n, cudaMemcpyDeviceToHost, 0));
+  CUDA_OK(ctx, cudaStreamSynchronize(0));
+  return MSPCG_OK;
+}
+
+// The same two calls with SINGLE-precision host vectors (ABI layout, float): for fp32 / fp16 computations the fp64 wire format doubles the
+// PCIe bytes of a step that is bound by them.  Device staging: the fp64 ABI buffers, used as float arrays.
+int mspcg_apply_MdagM_host32(mspcg_ctx* ctx, const float* in_host, float* out_host, int prec) {
+  int rc = check_ready(ctx, true); if (rc) return rc;
+  if (!in_host || !out_host || prec == MSPCG_F64 || !full_buf(ctx, prec)) return fail(ctx, MSPCG_EINVAL, "null pointer, or prec is fp64 / not configured (use mspcg_apply_MdagM_host)");
+  const size_t n = vec_bytes(ctx, MSPCG_F32, ctx->Ls);
+  float *din = (float*)ctx->abi_in, *dout = (float*)ctx->abi_out;
+  CUDA_OK(ctx, cudaMemcpyAsync(din, in_host, n, cudaMemcpyHostToDevice, 0));
+  CUDA_OK(ctx, pack_any_t<float>(ctx, din, ctx->stage_in, prec, 1, 0, 0));
+  CUDA_OK(ctx, normal_full_any(ctx, prec, ctx->stage_in, ctx->stage_out, nullptr, 0));
+  CUDA_OK(ctx, pack_any_t<float>(ctx, dout, ctx->stage_out, prec, 0, 0, 0));
+  CUDA_OK(ctx, cudaMemcpyAsync(out_host, dout, n, cudaMemcpyDeviceToHost, 0));
+  CUDA_OK(ctx, cudaStreamSynchronize(0));
+  return MSPCG_OK;
+}
+int mspcg_apply_precond_host32(mspcg_ctx* ctx, const float* r_host, float* z_host, int io_prec, int n_inner, int use_reduced) {
+  int rc = check_ready(ctx, true); if (rc) return rc;
+  if (!r_host || !z_host || n_inner < 1 || n_inner > KMAX || (io_prec != MSPCG_F32 && io_prec != MSPCG_F16)) return fail(ctx, MSPCG_EINVAL, "bad argument (io_prec fp32 or fp16, 1 <= n_inner <= %d)", KMAX);
+  if (use_reduced && !ctx->Ls_hat) return fail(ctx, MSPCG_EINVAL, "use_reduced without mspcg_set_reduced_ls");
+  const size_t n = vec_bytes(ctx, MSPCG_F32, ctx->Ls);
+  float *din = (float*)ctx->abi_in, *dout = (float*)ctx->abi_out;
+  CUDA_OK(ctx, cudaMemcpyAsync(din, r_host, n, cudaMemcpyHostToDevice, 0));
+  CUDA_OK(ctx, pack_any_t<float>(ctx, din, ctx->stage_in, io_prec, 1, 0, 0));
+  CUDA_OK(ctx, precond_any(ctx, ctx->stage_in, ctx->stage_out, io_prec, n_inner, use_reduced != 0, 0));
+  CUDA_OK(ctx, pack_any_t<float>(ctx, dout, ctx->stage_out, io_prec, 0, 0, 0));
+  CUDA_OK(ctx, cudaMemcpyAsync(z_host, dout, n, cudaMemcpyDeviceToHost, 0));
   CUDA_OK(ctx, cudaStreamSynchronize(0));
   return MSPCG_OK;
 }

@@ -9,7 +9,7 @@ import numpy as np
 import pytest
 
 from oracle.cbind import OracleC
-from paper_2104_05615_b200 import F16, F32, F64, LAYOUT_NATIVE, Mspcg, synth
+from paper_2104_05615_b200 import F16, F32, F64, LAYOUT_NATIVE, Mspcg, MspcgError, synth
 
 pytestmark = pytest.mark.gpu
 
@@ -258,6 +258,25 @@ def test_poisoned_neighbour_blocks_do_not_leak(inner):
         # equal up to the order of the atomic partial sums of the block's inner products
         assert rel(z_p[mask].cpu().numpy(), z_c[mask].cpu().numpy()) <= (1e-12 if inner == F64 else 2e-3)
         assert bool(torch.isnan(z_p[~mask]).any())            # the poison did reach the other blocks' own solves (the test has teeth)
+    g.close()
+
+
+def test_host32_entry_points_match_the_fp64_wire_format():
+    """mspcg_apply_*_host32 (float host vectors in the ABI layout) against the fp64 *_host calls and the oracle."""
+    dims, Ls, block, k = (4, 4, 6, 8), 8, (2, 2, 6, 4), 3
+    ora, g, torch = setup(dims, Ls, 0.02, block, outer=F32, inner=F16)
+    v = synth.gaussian_spinor_abi(dims, Ls, 12)
+    h64 = torch.as_tensor(v.reshape(-1)).pin_memory()
+    h32 = h64.to(torch.float32).pin_memory()
+    o64, o32 = torch.empty_like(h64).pin_memory(), torch.empty_like(h32).pin_memory()
+    g.apply_MdagM_host(h64, o64, F32)
+    g.apply_MdagM_host32(h32, o32, F32)
+    assert rel(o32.numpy(), o64.numpy()) <= 2e-7 and rel(o32.numpy(), ora.apply_MdagM(v)) <= 1e-5
+    g.apply_precond_host(h64, o64, k, F32)
+    g.apply_precond_host32(h32, o32, k, F32)
+    assert rel(o32.numpy(), o64.numpy()) <= 2e-3 and rel(o32.numpy(), ora.apply_precond(v, k)) <= 2e-2
+    with pytest.raises(MspcgError):
+        g.apply_MdagM_host32(h32, o32, F64)
     g.close()
 
 
