@@ -62,38 +62,14 @@ __device__ __forceinline__ uint2 lds64(uint32_t addr) {
   return v;
 }
 
-// Both half spinors of (1 + c gamma_mu) psi = (h, h'),  h = u + c G l,  h' = l + c G^dag u = c G^dag h  (G = -i sigma_k, 1 for
-// mu = t; c = -sg forward, +sg backward), are formed BEFORE the SU(3) product: upper += W h and lower += W h' are then two MMAs
-// with the same B fragment that accumulate over all eight directions, with no recombination arithmetic after the MMA
-// (hop_mma.cuh multiplies h only and maps W_b h_b - W_f h_f onto the lower components with 8 FMAs per direction pair and
-// segment).  chunk = {u0, l0, u1, l1}.
-template <int MU, bool FWD>
-__device__ __forceinline__ void project_lo(const uint4& q, const HsConst& k, uint32_t& h0, uint32_t& h1) {
-  if (MU == 0)      { const uint32_t m = FWD ? k.Q : k.R; h0 = hfma2_u32(swap_h2(q.z), m, q.y); h1 = hfma2_u32(swap_h2(q.x), m, q.w); }
-  else if (MU == 1) { h0 = hfma2_u32(q.z, FWD ? k.N : k.P, q.y); h1 = hfma2_u32(q.x, FWD ? k.P : k.N, q.w); }
-  else if (MU == 2) { h0 = hfma2_u32(swap_h2(q.x), FWD ? k.Q : k.R, q.y); h1 = hfma2_u32(swap_h2(q.z), FWD ? k.R : k.Q, q.w); }
-  else              { const uint32_t m = FWD ? k.N : k.P; h0 = hfma2_u32(q.x, m, q.y); h1 = hfma2_u32(q.z, m, q.w); }
-}
-template <int MU, int LS>
-__device__ __forceinline__ void hop_mu_full(float (&S)[MmaCfg<LS>::NMT][4], const uint4 (&F)[MmaCfg<LS>::NSEG], const uint4 (&B)[MmaCfg<LS>::NSEG],
-                                            uint32_t bf, uint32_t bb, const HsConst& k) {
-#pragma unroll
-  for (int seg = 0; seg < MmaCfg<LS>::NSEG; seg++) {
-    uint32_t f0, f1, b0, b1, g0, g1, c0, c1;
-    project_hs<MU, true>(F[seg], k, f0, f1);
-    project_hs<MU, false>(B[seg], k, b0, b1);
-    project_lo<MU, true>(F[seg], k, g0, g1);
-    project_lo<MU, false>(B[seg], k, c0, c1);
-    float (&S0)[4] = S[2 * seg], (&S1)[4] = S[2 * seg + 1];
-    mma16816_4(S0[0], S0[1], S1[0], S1[1], f0, f1, b0, b1, bf, bb);
-    mma16816_4(S0[2], S0[3], S1[2], S1[3], g0, g1, c0, c1, bf, bb);
-  }
-}
-// The same with the lower half spinor taken from the upper one: h' = c G^dag h, and G^dag = i sigma_k is a permutation of the two spin rows
+// (1 + c gamma_mu) psi = (h, h') with the half spinors h = u + c G l and h' = l + c G^dag u = c G^dag h  (G = -i sigma_k, 1 for mu = t;
+// c = -sg forward, +sg backward; chunk = {u0, l0, u1, l1}).  h is formed in the lane (project_hs, hop_mma.cuh) and is the A fragment of
+// upper += W h.  The lower half spinor is taken from the upper one: h' = c G^dag h, and G^dag = i sigma_k is a permutation of the two spin rows
 // times a phase, so  lower += W h' = (c phase W) (rows of h permuted, one row negated for mu = y, z):  the phase and the sign c go into a
 // second B fragment of the link (vf, vb: one byte permute each per direction and SITE), the row permutation is a choice of registers.
 //   mu = x: h' = c i (h1, h0)    mu = y: h' = c (h1, -h0)    mu = z: h' = c i (h0, -h1)    mu = t: h' = c (h0, h1)
-// 32 packed fp16 FMAs and 16 permutes per site column less than hop_mu_full, and h' is exact given h.
+// Against projecting both half spinors in the lane this saves 32 packed fp16 FMAs and 16 permutes per site column, against mapping
+// W_b h_b - W_f h_f onto the lower components after the MMA (hop_mma.cuh) 64 FMAs; h' is exact given h.
 template <int MU, int LS>
 __device__ __forceinline__ void hop_mu_perm(float (&S)[MmaCfg<LS>::NMT][4], const uint4 (&F)[MmaCfg<LS>::NSEG], const uint4 (&B)[MmaCfg<LS>::NSEG],
                                             uint32_t bf, uint32_t bb, uint32_t vf, uint32_t vb, const HsConst& k) {
@@ -142,9 +118,6 @@ __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const
     // Warp w fetches the input slots [w NIN/NWP, (w+1) NIN/NWP) (a lane issues a copy for each of its slots where a run starts)
     // and the link records of the output sites [w TS/NWP, (w+1) TS/NWP); warp 0 also fetches the tile header.  Every producer warp posts
     // the bytes of its own copies on the stage's `full` barrier (arrival count NWP) before it issues them.
-#ifdef MSPCG_TILE_PURE
-    return;
-#endif
     int stage = 0, blk = blk0, ti = ti0;
     uint32_t phases = 0xffffffffu;   // bit s: parity to wait for on empty[s]; a fresh barrier passes a wait on the phase before its first one
     constexpr int SPW = TC::NIN / TC::NWP / 32;        // input slots per lane
@@ -235,30 +208,20 @@ __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const
     if (EPI == EPI_XPAY && a.dot_out) dot4 = reinterpret_cast<const uint4*>(a.dotv) + (long)blk * a.dotv_stride * (LS * 3);
 
     const uint32_t sb = sm_u32 + stage * TC::STAGE;
-#ifndef MSPCG_TILE_PURE
     mbar_wait(full_u32 + 8 * stage, (phases >> stage) & 1u);
-#endif
     const uint32_t hdr = sb + TC::OFF_HDR;
     const uint4* stg4 = reinterpret_cast<const uint4*>(smraw + stage * TC::STAGE);
     const uint32_t* lk32 = reinterpret_cast<const uint32_t*>(smraw + stage * TC::STAGE + TC::OFF_LINK);
     const uint32_t* zero32 = reinterpret_cast<const uint32_t*>(smraw + stage * TC::STAGE + TC::OFF_ZERO);
-#ifdef MSPCG_TILE_PURE
-    const int n_out = 32;
-#else
     const int n_out = (int)lds32(hdr);
-#endif
     // One output site in three pieces, so that two sites can be worked on in the same straight-line code (TC::PAIR, below).  Measured at C2
     // (DESIGN.md section 4): 12 consumer warps x 2 sites per warp run exactly as fast as 16 x 1 (K2/K4 0.0727 vs 0.0723 ms), as do 20 and 24
     // warps at 80 / 72 registers -- the kernel is bound by its per-site instruction stream on the ALU / FMA pipes, not by latency.
     struct SiteCtx { int site; uint2 sl; unsigned have; uint4 av[NSEG], dv[NSEG]; float S[NMT][4]; const uint32_t* lkb; };
     auto begin = [&](SiteCtx& x, const int j) {
-#ifdef MSPCG_TILE_PURE
-      x.site = (int)(((long)ti * 32 + j) % a.n_out); x.sl = make_uint2(0x03020100u + 0x04040404u * (j & 15), 0x07060504u + 0x04040404u * (j & 15)); x.have = 0xffu;
-#else
       x.site = (int)lds32(hdr + 16 + 4 * j);
       x.sl = lds64(hdr + 16 + 4 * TC::TS + 8 * j);
       x.have = (lds32(hdr + 16 + 12 * TC::TS + (j & ~3)) >> (8 * (j & 3))) & 0xffu;
-#endif
       if (EPI != EPI_PLAIN) {
         const bool ok = x.site < a.n_aux;
         const uint4* p = aux4 + (long)x.site * (LS * 3);
@@ -340,11 +303,7 @@ __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const
     typedef std::integral_constant<int, 2> M2; typedef std::integral_constant<int, 3> M3;
     // sites are dealt to the consumer warps round robin, continuing across tiles (tile sizes are not multiples of NWC)
     int j = cw >= rot ? cw - rot : cw - rot + NWC;
-#ifdef MSPCG_TILE_PURE
-    if (true) {
-#else
     if (lds32(hdr + 8) != 0u) {
-#endif
       // every site of the tile has all eight neighbours (flag in the tile header): no branches, two sites at a time
       for (; TC::PAIR && j + NWC < n_out; j += 2 * NWC) {
         SiteCtx x0, x1;
@@ -373,9 +332,7 @@ __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const
     }
     rot = (rot + n_out) % NWC;
     __syncwarp();
-#ifndef MSPCG_TILE_PURE
     if (lane == 0) mbar_arrive(empty_u32 + 8 * stage);
-#endif
     phases ^= 1u << stage;
     stage = stage + 1 == TC::NSTAGE ? 0 : stage + 1;
     if (++ti == a.n_tiles) { ti = 0; blk++; }
