@@ -214,6 +214,21 @@ long mspcg_launch_count(const mspcg_ctx* ctx);
 int mspcg_timing(mspcg_ctx* ctx, int enable);
 int mspcg_timing_read(mspcg_ctx* ctx, double* ms_host, long* launches_host);
 
+/* The two inner products of the Polak-Ribiere beta (eq. 18, R16) WITHOUT a context, a workspace or any allocation:
+ * for callers that cannot call cudaMalloc (code under CUDA graph capture, serving loops).  out_dev[0] = sum_i a[i] b[i],
+ * out_dev[1] = sum_i a[i] c[i] (0 if c_dev is NULL) over n_reals doubles; a_dev, b_dev, c_dev (DEVICE, fp64, any layout: the sum runs over all
+ * reals; a == b gives |a|^2), out_dev (DEVICE, 2 doubles, caller-owned).  Stream-ordered on `stream`, no synchronisation, no
+ * cudaMalloc / cudaFree / allocating library call; one cudaMemsetAsync (4 bytes) and one kernel.  The partial sums (one pair per 16384
+ * reals) and a ticket counter live in a file-scope device array of 513 KiB that every GPU holds from the time the library is loaded until
+ * exit; hence n_reals <= mspcg_dot2_noalloc_max_reals() = 2^29 (a 4 GiB vector; C1..C4 fit, C5 does not).  The sums are added in a fixed
+ * order: the result does not depend on the grid or on scheduling (bitwise equal from call to call).  ALL calls on a device share the
+ * array: calls that overlap on the GPU (different streams without an ordering between them, or several host threads) RACE; calls on
+ * one stream, or otherwise ordered, do not.  Errors: MSPCG_EINVAL (null out; null a or b with n_reals > 0; n_reals < 0 or above the maximum), MSPCG_ECUDA;
+ * the message is mspcg_noalloc_last_error() (per host thread). */
+int mspcg_dot2_noalloc(const double* a_dev, const double* b_dev, const double* c_dev, long n_reals, double* out_dev, void* stream);
+long mspcg_dot2_noalloc_max_reals(void);
+const char* mspcg_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -5,4 +5,4 @@ it and `synth` makes the seeded synthetic inputs shared with the CPU oracle (whi
 infrastructure only).
 """
 from . import synth  # noqa: F401
-from .binding import (F16, F32, F64, LAYOUT_ABI, LAYOUT_NATIVE, Mspcg, MspcgError, load_library)  # noqa: F401
+from .binding import (F16, F32, F64, LAYOUT_ABI, LAYOUT_NATIVE, Mspcg, MspcgError, dot2_noalloc, load_library)  # noqa: F401

@@ -25,6 +25,7 @@ SYMBOLS = [
     "mspcg_apply_precond_host", "mspcg_apply_A_block", "mspcg_set_reduced_ls", "mspcg_solve", "mspcg_launch_count",
     "mspcg_timing", "mspcg_timing_read", "mspcg_update_T", "mspcg_train_eval", "mspcg_train_T",
     "mspcg_prepare_source", "mspcg_reconstruct_odd", "mspcg_apply_full", "mspcg_apply_M5inv", "mspcg_residual", "mspcg_set_block_group", "mspcg_tile_check", "mspcg_apply_MdagM_host32", "mspcg_apply_precond_host32",
+    "mspcg_dot2_noalloc", "mspcg_dot2_noalloc_max_reals", "mspcg_noalloc_last_error",
 ]
 
 
@@ -88,6 +89,11 @@ def load_library():
     L.mspcg_train_T.argtypes = [vp, vp, i, i, i, d, dp, dp, vp]
     L.mspcg_timing.argtypes = [vp, i]
     L.mspcg_timing_read.argtypes = [vp, dp, C.POINTER(C.c_long)]
+    L.mspcg_dot2_noalloc.argtypes = [vp, vp, vp, C.c_long, vp, vp]
+    L.mspcg_dot2_noalloc_max_reals.argtypes = []
+    L.mspcg_dot2_noalloc_max_reals.restype = C.c_long
+    L.mspcg_noalloc_last_error.argtypes = []
+    L.mspcg_noalloc_last_error.restype = C.c_char_p
     _lib = L
     return L
 
@@ -111,6 +117,23 @@ def _torch():
 def _dtype(prec):
     torch = _torch()
     return {F64: torch.float64, F32: torch.float32, F16: torch.float16}[prec]
+
+
+def dot2_noalloc(a, b, c, out):
+    """mspcg_dot2_noalloc: out[0] = <a,b>, out[1] = <a,c> (c may be None) over all reals of the fp64 CUDA tensors a, b, c, into the
+    caller's 2-element fp64 CUDA tensor `out`, on torch's current stream.  Allocates nothing (the library's static scratch array)."""
+    torch = _torch()
+    lib = load_library()
+    for t in (a, b, out) + ((c,) if c is not None else ()):
+        if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+            raise ValueError("dot2_noalloc wants contiguous fp64 CUDA tensors")
+    if b.numel() != a.numel() or (c is not None and c.numel() != a.numel()) or out.numel() < 2:
+        raise ValueError("dot2_noalloc: size mismatch")
+    rc = lib.mspcg_dot2_noalloc(C.c_void_p(a.data_ptr()), C.c_void_p(b.data_ptr()), C.c_void_p(c.data_ptr() if c is not None else None),
+                                a.numel(), C.c_void_p(out.data_ptr()), C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    if rc != 0:
+        raise MspcgError(rc, lib.mspcg_noalloc_last_error().decode())
+    return out
 
 
 class Mspcg:

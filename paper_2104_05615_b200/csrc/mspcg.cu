@@ -10,6 +10,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <type_traits>
 #include <string>
@@ -1486,6 +1487,115 @@ int mspcg_timing_read(mspcg_ctx* ctx, double* ms_host, long* launches_host) {
     ms_host[ctx->ev_cls[i]] += ms; launches_host[ctx->ev_cls[i]]++;
   }
   ctx->ev_used = 0; ctx->ev_cls.clear();
+  return MSPCG_OK;
+}
+
+}  // extern "C"
+
+// ======================================================================================================================
+// mspcg_dot2_noalloc: the two inner products of the Polak-Ribiere beta (eq. 18, R16; k_dot2 in kernels.cuh) for callers
+// that cannot allocate (CUDA graph capture, serving loops): no context, no workspace.  k_dot2 accumulates with atomics into
+// scratch scalars of the caller's workspace; this variant keeps its scratch -- one pair of partial sums per CHUNK of the
+// vectors and a ticket counter -- in the file-scope device array below, which every GPU that loads the library holds until
+// exit (NOALLOC_BYTES = 513 KiB).  The result does not depend on the grid size or on the order in which thread blocks finish.
+// ======================================================================================================================
+namespace {
+
+constexpr long NOALLOC_CHUNK = 16384;                 // reals per partial sum (one thread block pass)
+constexpr long NOALLOC_MAX_CHUNKS = 32768;            // => at most 2^29 reals (4 GiB of fp64) per vector
+constexpr long NOALLOC_MAX_REALS = NOALLOC_CHUNK * NOALLOC_MAX_CHUNKS;
+constexpr size_t NOALLOC_BYTES = sizeof(double) * 2 * NOALLOC_MAX_CHUNKS + 256;   // partial sums, then the ticket counter
+constexpr int NOALLOC_MAX_DEVICES = 64;
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NOALLOC_BYTES];
+
+// grid-stride over chunks; partial[2 c], partial[2 c + 1] = <a,b>, <a,c> over chunk c, summed in a fixed order; the thread block
+// that draws the last ticket adds the partial sums in a fixed order and writes out[0..1].
+__global__ void __launch_bounds__(256) k_dot2_static(const double* __restrict__ a, const double* __restrict__ b, const double* __restrict__ c,
+                                                     long n, long nchunks, double* partial, unsigned int* ticket, double* out) {
+  __shared__ double red[32];
+  __shared__ bool last;
+  for (long ch = blockIdx.x; ch < nchunks; ch += gridDim.x) {
+    const long lo = ch * NOALLOC_CHUNK, hi = lo + NOALLOC_CHUNK < n ? lo + NOALLOC_CHUNK : n;
+    double p0 = 0, p1 = 0;
+    for (long i = lo + threadIdx.x; i < hi; i += 256) {
+      const double va = a[i];
+      p0 += va * b[i];
+      if (c) p1 += va * c[i];
+    }
+    const double t0 = block_sum(p0, red, threadIdx.x, 256);
+    __syncthreads();
+    const double t1 = block_sum(p1, red, threadIdx.x, 256);
+    __syncthreads();
+    if (threadIdx.x == 0) { partial[2 * ch] = t0; partial[2 * ch + 1] = t1; }
+  }
+  if (threadIdx.x == 0) {
+    __threadfence();
+    last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+  }
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  double s0 = 0, s1 = 0;
+  for (long ch = threadIdx.x; ch < nchunks; ch += 256) { s0 += __ldcg(partial + 2 * ch); s1 += __ldcg(partial + 2 * ch + 1); }
+  const double t0 = block_sum(s0, red, threadIdx.x, 256);
+  __syncthreads();
+  const double t1 = block_sum(s1, red, threadIdx.x, 256);
+  if (threadIdx.x == 0) { out[0] = t0; out[1] = t1; *ticket = 0; }
+}
+
+std::mutex g_noalloc_mu;
+unsigned char* g_noalloc_ptr[NOALLOC_MAX_DEVICES];    // device address of g_noalloc_scratch on each device (host code cannot use the symbol's name as a pointer)
+int g_noalloc_sms[NOALLOC_MAX_DEVICES];
+thread_local char g_noalloc_err[256] = "";
+
+int noalloc_fail(int code, const char* fmt, ...) {
+  va_list ap; va_start(ap, fmt); vsnprintf(g_noalloc_err, sizeof(g_noalloc_err), fmt, ap); va_end(ap);
+  return code;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* mspcg_noalloc_last_error(void) { return g_noalloc_err; }
+long mspcg_dot2_noalloc_max_reals(void) { return NOALLOC_MAX_REALS; }
+
+int mspcg_dot2_noalloc(const double* a_dev, const double* b_dev, const double* c_dev, long n_reals, double* out_dev, void* stream) {
+  if (!out_dev || (n_reals > 0 && (!a_dev || !b_dev))) return noalloc_fail(MSPCG_EINVAL, "mspcg_dot2_noalloc: null pointer");
+  if (n_reals < 0 || n_reals > NOALLOC_MAX_REALS)
+    return noalloc_fail(MSPCG_EINVAL, "mspcg_dot2_noalloc: n_reals = %ld is outside [0, %ld] (the static scratch holds %ld partial sums of %ld reals)",
+                        n_reals, NOALLOC_MAX_REALS, NOALLOC_MAX_CHUNKS, NOALLOC_CHUNK);
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return noalloc_fail(MSPCG_ECUDA, "mspcg_dot2_noalloc: cudaGetDevice: %s", cudaGetErrorString(e));
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return noalloc_fail(MSPCG_EINVAL, "mspcg_dot2_noalloc: device ordinal %d >= %d", dev, NOALLOC_MAX_DEVICES);
+  unsigned char* base; int sms;
+  {   // once per device, with that device current: the device address of the scratch array
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_ptr[dev]) {
+      void* p = nullptr;
+      e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+      if (e != cudaSuccess || !p) return noalloc_fail(MSPCG_ECUDA, "mspcg_dot2_noalloc: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+      int n = 0;
+      e = cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+      if (e != cudaSuccess || n < 1) return noalloc_fail(MSPCG_ECUDA, "mspcg_dot2_noalloc: cudaDeviceGetAttribute: %s", cudaGetErrorString(e));
+      g_noalloc_sms[dev] = n;
+      g_noalloc_ptr[dev] = (unsigned char*)p;
+    }
+    base = g_noalloc_ptr[dev]; sms = g_noalloc_sms[dev];
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  double* partial = reinterpret_cast<double*>(base);
+  unsigned int* ticket = reinterpret_cast<unsigned int*>(base + sizeof(double) * 2 * NOALLOC_MAX_CHUNKS);
+  // the array keeps the last call's contents: the ticket must start at zero (the partial sums are overwritten before they are read)
+  e = cudaMemsetAsync(ticket, 0, sizeof(unsigned int), st);
+  if (e != cudaSuccess) return noalloc_fail(MSPCG_ECUDA, "mspcg_dot2_noalloc: cudaMemsetAsync: %s", cudaGetErrorString(e));
+  const long nchunks = (n_reals + NOALLOC_CHUNK - 1) / NOALLOC_CHUNK;
+  const long want = nchunks < 1 ? 1 : nchunks, cap = 8L * sms;
+  k_dot2_static<<<(unsigned)(want < cap ? want : cap), 256, 0, st>>>(a_dev, b_dev, c_dev, n_reals, nchunks, partial, ticket, out_dev);
+  e = cudaPeekAtLastError();
+  if (e != cudaSuccess) return noalloc_fail(MSPCG_ECUDA, "mspcg_dot2_noalloc: launch: %s", cudaGetErrorString(e));
   return MSPCG_OK;
 }
 
