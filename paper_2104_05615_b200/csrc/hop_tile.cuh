@@ -16,8 +16,8 @@
 //     mma.m16n8k16, fp32 accumulation); neighbour fragments are 128-bit shared-memory reads at slot * column size;
 //     link words are 32-bit shared-memory reads; a consumer touches global memory only for the xpay / dot operands
 //     and for its stores.  When a warp is done with a stage it arrives on the stage's `empty` mbarrier.
-// Tiles are dealt to thread blocks in contiguous chunks of the flattened (Dirichlet block, tile) index, so a thread block
-// stays inside one Dirichlet block for many tiles (one atomic per warp and Dirichlet block for the fused <p, A p>).
+// Tiles are dealt to thread blocks round robin over the flattened (Dirichlet block, tile) index (neighbouring cells are in
+// flight at the same time: L2 reuse); the fused <p, A p> costs one atomic per warp and tile.
 // Links carry the antiperiodic sign already (18 reals; the 12-real format keeps the per-warp kernel).
 #pragma once
 #include <type_traits>
@@ -50,6 +50,9 @@ template <int LS, int EPI = 0> struct TileCfg {
 
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;\n" ::"l"(src), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
   uint32_t v;
@@ -87,16 +90,38 @@ __device__ __forceinline__ void hop_mu_perm(float (&S)[MmaCfg<LS>::NMT][4], cons
   }
 }
 
+// dense5d_mma (hop_mma.cuh) with the A fragments of the two chirality blocks in registers instead of shared memory
+template <int LS>
+__device__ __forceinline__ void dense5d_mma_reg(float (&X)[MmaCfg<LS>::NMT][4], const uint4& A0, const uint4& A1) {
+  typedef MmaCfg<LS> Cfg;
+#pragma unroll
+  for (int hi = 0; hi < 2; hi++) {
+    const uint4& A = hi ? A1 : A0;
+#pragma unroll
+    for (int sp = 0; sp < 2; sp++) {
+      const uint32_t b0 = movmatrix_trans(pack_h2(X[sp][2 * hi], X[sp][2 * hi + 1]));
+      uint32_t b1 = 0u;
+      if (Cfg::NSEG == 2) b1 = movmatrix_trans(pack_h2(X[Cfg::NMT - 2 + sp][2 * hi], X[Cfg::NMT - 2 + sp][2 * hi + 1]));
+      float d[4] = {0.f, 0.f, 0.f, 0.f};
+      mma16816(d, A.x, A.y, A.z, A.w, b0, b1);
+      X[sp][2 * hi] = d[0]; X[sp][2 * hi + 1] = d[1];
+      if (Cfg::NSEG == 2) { X[Cfg::NMT - 2 + sp][2 * hi] = d[2]; X[Cfg::NMT - 2 + sp][2 * hi + 1] = d[3]; }
+    }
+  }
+}
+
 template <int LS, int EPI>
 __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const HopArgs<__half> a) {
   typedef MmaCfg<LS> Cfg;
   typedef TileCfg<LS, EPI> TC;
   constexpr int NSEG = Cfg::NSEG, NMT = Cfg::NMT, NWC = TC::NWC;
   extern __shared__ __align__(128) unsigned char smraw[];
-  __shared__ uint4 sfrag[(EPI == EPI_K3 ? 2 : 1) * 64];   // A fragments of the 5D matrices
+  __shared__ uint4 sfrag[EPI == EPI_K3 ? 128 : 64];       // A fragments of the 5D matrices (kernels 2 and 4 keep theirs in registers; the others have none to spare)
   __shared__ __align__(8) uint64_t bars[2 * TC::NSTAGE];  // full[stage], empty[stage]
-  if (threadIdx.x < 64) sfrag[threadIdx.x] = __ldg(a.frag1 + threadIdx.x);
-  if (EPI == EPI_K3) { if (threadIdx.x >= 64 && threadIdx.x < 128) sfrag[threadIdx.x] = __ldg(a.frag2 + threadIdx.x - 64); }
+  if (EPI != EPI_PLAIN) {
+    if (threadIdx.x < 64) sfrag[threadIdx.x] = __ldg(a.frag1 + threadIdx.x);
+    else if (EPI == EPI_K3 && threadIdx.x < 128) sfrag[threadIdx.x] = __ldg(a.frag2 + threadIdx.x - 64);
+  }
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t sm_u32 = smem_u32(smraw);
   const uint32_t full_u32 = smem_u32(bars), empty_u32 = full_u32 + 8 * TC::NSTAGE;
@@ -107,23 +132,25 @@ __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const
   }
   __syncthreads();
 
+  // Thread block b takes the tiles b, b + gridDim.x, ... of the flattened (Dirichlet block, tile) index: at any time the resident thread
+  // blocks work on ~gridDim.x CONSECUTIVE tiles, i.e. on neighbouring cells, so a column shared by two tiles is fetched by both within
+  // a few microseconds and the second fetch hits L2 (measured at C2 against contiguous chunks per thread block: DRAM reads -13 .. -22 %,
+  // kernel time -3 .. -5 %, profiles/r2_hop_tile_whatif.md).
   const long total = (long)a.nblk * a.n_tiles;
-  const long per = (total + gridDim.x - 1) / gridDim.x;
-  const long t_begin = (long)blockIdx.x * per;
-  const long t_end = t_begin + per < total ? t_begin + per : total;
+  const long t_begin = blockIdx.x, t_step = gridDim.x;
 
-  int blk0 = (int)(t_begin / a.n_tiles), ti0 = (int)(t_begin - (long)blk0 * a.n_tiles);
   if (warp < TC::NWP) {
     // ----------------------------------------------------------------------------------------------- producer warps
     // Warp w fetches the input slots [w NIN/NWP, (w+1) NIN/NWP) (a lane issues a copy for each of its slots where a run starts)
     // and the link records of the output sites [w TS/NWP, (w+1) TS/NWP); warp 0 also fetches the tile header.  Every producer warp posts
     // the bytes of its own copies on the stage's `full` barrier (arrival count NWP) before it issues them.
-    int stage = 0, blk = blk0, ti = ti0;
+    int stage = 0;
     uint32_t phases = 0xffffffffu;   // bit s: parity to wait for on empty[s]; a fresh barrier passes a wait on the phase before its first one
     constexpr int SPW = TC::NIN / TC::NWP / 32;        // input slots per lane
     constexpr int OPW = TC::TS / TC::NWP;              // output sites per producer warp
     const int slot0 = (TC::NIN / TC::NWP) * warp + lane, oj = OPW * warp + (lane < OPW ? lane : 0);
-    for (long tt = t_begin; tt < t_end; tt++) {
+    for (long tt = t_begin; tt < total; tt += t_step) {
+      const int blk = (int)(tt / a.n_tiles), ti = (int)(tt - (long)blk * a.n_tiles);
       const TileRec* rec = a.tiles + ti;
       int col[SPW]; uint32_t run[SPW], nrun = 0;
 #pragma unroll
@@ -145,9 +172,15 @@ __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const
       if (orun)
         bulk_g2s(sb + TC::OFF_LINK + oj * TC::LINKREC,
                  reinterpret_cast<const unsigned char*>(a.links) + ((long)blk * a.link_stride + osite) * TC::LINKREC, orun * TC::LINKREC, bar);
+      // kernel 3's consumers read the xpay operand of the output sites straight from global memory about one tile later: pull it into L2 now
+      // (measured at C2: kernel 3 -4 %; the same for kernel 5's two operands changes nothing, and prefetching the NEXT tile's columns makes
+      // every kernel slower, +3 .. +15 %: profiles/r2_hop_tile_whatif.md)
+      if (EPI == EPI_K3 && orun) {
+        const int n = osite + (int)orun <= a.n_aux ? (int)orun : a.n_aux - osite;
+        if (n > 0) bulk_prefetch_l2(reinterpret_cast<const unsigned char*>(a.aux) + ((long)blk * a.aux_stride + osite) * TC::COL, n * TC::COL);
+      }
       phases ^= 1u << stage;
       stage = stage + 1 == TC::NSTAGE ? 0 : stage + 1;
-      if (++ti == a.n_tiles) { ti = 0; blk++; }
     }
     return;
   }
@@ -177,6 +210,8 @@ __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const
   const uint32_t vsel_f02 = sgp ? sel_im : sel_ip, vsel_b02 = sgp ? sel_ip : sel_im;  // mu = x, z: c i W
   const int lk_step = lk_mine ? 9 : 0;
 
+  uint4 rA0 = make_uint4(0, 0, 0, 0), rA1 = rA0;
+  if (EPI == EPI_PLAIN) { rA0 = __ldg(a.frag1 + lane); rA1 = __ldg(a.frag1 + 32 + lane); }
   float part = 0.f;
   int part_blk = -1;
   auto flush_dot = [&]() {
@@ -197,8 +232,9 @@ __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const
     }
     asm volatile("bar.sync 1, %0;\n" ::"n"(32 * NWC) : "memory");   // consumer warps only
   }
-  int blk = blk0, ti = ti0, rot = 0;
-  for (long tt = t_begin; tt < t_end; tt++) {
+  int rot = 0;
+  for (long tt = t_begin; tt < total; tt += t_step) {
+    const int blk = (int)(tt / a.n_tiles);
     if (blk != part_blk) { flush_dot(); part_blk = blk; }
     const uint4* aux4 = nullptr; const uint4* dot4 = nullptr;
     uint4* out4 = reinterpret_cast<uint4*>(a.out) + (long)blk * a.out_stride * (LS * 3);
@@ -259,7 +295,8 @@ __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const
     auto finish = [&](SiteCtx& x) {
       float (&S)[NMT][4] = x.S;
       const int site = x.site;
-      dense5d_mma<LS>(S, sfrag, lane);
+      if (EPI == EPI_PLAIN) dense5d_mma_reg<LS>(S, rA0, rA1);
+      else dense5d_mma<LS>(S, sfrag, lane);
       uint4 o[NSEG];
       uint4* po = out4 + (long)site * (LS * 3);
       if (EPI == EPI_PLAIN) {
@@ -335,7 +372,6 @@ __global__ void __launch_bounds__(TileCfg<LS, EPI>::THREADS, 1) k_hop_tile(const
     if (lane == 0) mbar_arrive(empty_u32 + 8 * stage);
     phases ^= 1u << stage;
     stage = stage + 1 == TC::NSTAGE ? 0 : stage + 1;
-    if (++ti == a.n_tiles) { ti = 0; blk++; }
   }
   flush_dot();
 }
