@@ -194,6 +194,21 @@ int mspcg_residual(mspcg_ctx* ctx, const double* b_dev, const double* x_dev, dou
  * interact, R13).  The environment variable MSPCG_GROUP sets the default of new contexts.  Errors: MSPCG_EINVAL (G < 0). */
 int mspcg_set_block_group(mspcg_ctx* ctx, int blocks_per_group);
 
+/* Fixed-point storage of PAPER.md:268-285 eq. 17 (reading R21: integer-limit 2^(bits-1) - 1, scale = largest |real| of the
+ * colour-spinor's 24 numbers in fp32, integer = round-half-even(x / scale * limit) in fp32).
+ * mspcg_fixed_pack / _unpack: the format itself.  abi_dev (DEVICE, fp64, ABI layout, Ls*V4/2*24 doubles) <-> q_dev (DEVICE, Ls*V4/2*24 signed
+ * integers of `bits` = 8 or 16 bits, same order) and scale_dev (DEVICE, Ls*V4/2 floats, one per colour-spinor (s, x_cb)); unpack returns
+ * integer / limit * scale evaluated in fp32.  Need no workspace and no gauge field.  Integers and scales are bit-identical to the oracle's.
+ * mspcg_set_fixed_storage(bits = 8 | 16): the full-Ls preconditioner with fp32 inner storage (inner_prec = MSPCG_F32) passes every vector its
+ * inner CG writes -- r, p, q = A p, x ("the matrix multiplication and BLAS operations use the 8-bit and 16-bit fixed-point
+ * formats") -- through that store, inside the kernels that write them; <p, q> and |r|^2 are taken from the stored values.  The VALUES are those
+ * of fixed-point storage; the bytes in HBM stay fp32 (a numerics mode for the paper's 8- vs 16-bit comparison, not a bandwidth one: DESIGN.md
+ * section 9 says why the tensor-core hop cannot use the format).  bits = 0 (default): off.  Ignored by fp16 / fp64 inner storage and by the
+ * reduced-Ls preconditioner.  Errors: MSPCG_EINVAL (null pointer, bits not in the list). */
+int mspcg_fixed_pack(mspcg_ctx* ctx, const double* abi_dev, void* q_dev, float* scale_dev, int bits, void* stream);
+int mspcg_fixed_unpack(mspcg_ctx* ctx, const void* q_dev, const float* scale_dev, double* abi_dev, int bits, void* stream);
+int mspcg_set_fixed_storage(mspcg_ctx* ctx, int bits);
+
 /* Host-only self check of the site tiles of the fp16 tile kernel (hop_tile.cuh; needs no GPU and no workspace): builds the tile tables of
  * the Dirichlet-block and the full-lattice geometry and verifies them against the neighbour tables (every output site in exactly one
  * tile, every neighbour's shared-memory slot holding that neighbour's column, absent neighbours on the zero column, copy runs consecutive

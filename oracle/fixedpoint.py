@@ -83,3 +83,20 @@ def cg_fixed_stored(apply_A, r_in, k, bits):
         p = store(r + (rho_new / rho) * p, bits)
         rho = rho_new
     return x, napply
+
+
+def precond_fixed(pre, r_full, k, bits, blocks=None):
+    """z = M^-1 r (eq. 12-14, PAD reading R10) with the vectors of every block's k-step CG in fixed-point storage
+    (cg_fixed_stored above).  `pre` is a solvers.BlockPrecond (variant PAD): its padded boxes and block operator are used as they are."""
+    from . import mdwf
+    if pre.variant != "PAD":
+        raise ValueError("precond_fixed follows the PAD reading (R10)")
+    z = np.zeros_like(r_full)
+    todo = pre.origins if blocks is None else [pre.origins[i] for i in blocks]
+    for o in todo:
+        Ub, per = pre._box(o)
+        rb = mdwf.box_embed(r_full, pre.dims, pre.block, o)
+        xb, n = cg_fixed_stored(lambda p: mdwf.A_block_pad(pre.mob, Ub, per, p, pre.centre), rb, k, bits)
+        mdwf.box_extract_add(z, xb, pre.dims, pre.block, o)
+        pre.napply += n
+    return z

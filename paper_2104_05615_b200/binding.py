@@ -26,6 +26,7 @@ SYMBOLS = [
     "mspcg_timing", "mspcg_timing_read", "mspcg_update_T", "mspcg_train_eval", "mspcg_train_T",
     "mspcg_prepare_source", "mspcg_reconstruct_odd", "mspcg_apply_full", "mspcg_apply_M5inv", "mspcg_residual", "mspcg_set_block_group", "mspcg_tile_check", "mspcg_apply_MdagM_host32", "mspcg_apply_precond_host32",
     "mspcg_dot2_noalloc", "mspcg_dot2_noalloc_max_reals", "mspcg_noalloc_last_error",
+    "mspcg_fixed_pack", "mspcg_fixed_unpack", "mspcg_set_fixed_storage",
 ]
 
 
@@ -89,6 +90,9 @@ def load_library():
     L.mspcg_train_T.argtypes = [vp, vp, i, i, i, d, dp, dp, vp]
     L.mspcg_timing.argtypes = [vp, i]
     L.mspcg_timing_read.argtypes = [vp, dp, C.POINTER(C.c_long)]
+    L.mspcg_fixed_pack.argtypes = [vp, vp, vp, vp, i, vp]
+    L.mspcg_fixed_unpack.argtypes = [vp, vp, vp, vp, i, vp]
+    L.mspcg_set_fixed_storage.argtypes = [vp, i]
     L.mspcg_dot2_noalloc.argtypes = [vp, vp, vp, C.c_long, vp, vp]
     L.mspcg_dot2_noalloc_max_reals.argtypes = []
     L.mspcg_dot2_noalloc_max_reals.restype = C.c_long
@@ -313,6 +317,25 @@ class Mspcg:
     def set_block_group(self, blocks_per_group):
         """L2-resident groups of Dirichlet blocks for the preconditioner (mspcg_set_block_group); 0 = all blocks at once."""
         self._check(self.lib.mspcg_set_block_group(self.h, int(blocks_per_group)))
+
+    def set_fixed_storage(self, bits):
+        """fp32 inner CG vectors pass through the 8- / 16-bit fixed-point store of eq. 17 (mspcg_set_fixed_storage); 0 = off."""
+        self._check(self.lib.mspcg_set_fixed_storage(self.h, int(bits)))
+
+    def fixed_pack(self, v_abi, bits):
+        """ABI vector -> (integers [Ls*V/2*24] int8 / int16, scales [Ls*V/2] float32) in the fixed-point format of eq. 17 (mspcg_fixed_pack)."""
+        torch = _torch()
+        n = v_abi.numel() // 24
+        q = torch.empty(n * 24, dtype=torch.int8 if bits == 8 else torch.int16, device="cuda")
+        sc = torch.empty(n, dtype=torch.float32, device="cuda")
+        self._check(self.lib.mspcg_fixed_pack(self.h, C.c_void_p(v_abi.data_ptr()), C.c_void_p(q.data_ptr()), C.c_void_p(sc.data_ptr()), int(bits), self._stream()))
+        return q, sc
+
+    def fixed_unpack(self, q, sc, bits):
+        torch = _torch()
+        out = torch.empty(q.numel(), dtype=torch.float64, device="cuda")
+        self._check(self.lib.mspcg_fixed_unpack(self.h, C.c_void_p(q.data_ptr()), C.c_void_p(sc.data_ptr()), C.c_void_p(out.data_ptr()), int(bits), self._stream()))
+        return out
 
     def residual(self, b_abi, x_abi, normalise=False):
         """r = b - D^dag D x in fp64 (mspcg_residual), optionally divided by its norm; returns (r, |b - D^dag D x|)."""

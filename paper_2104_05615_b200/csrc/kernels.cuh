@@ -328,6 +328,22 @@ __global__ void __launch_bounds__(Tile<LS>::NT, (sizeof(typename ST<T>::C) == 8 
 #include "hop_tile.cuh"
 namespace mspcg {
 
+// Fixed-point storage of PAPER.md:268-285 eq. 17 (reading R21) applied to the 24 reals of ONE colour-spinor, which is what a thread of the
+// BLAS-1 kernels holds: v becomes what an 8- / 16-bit store of it returns,  integer / limit * scale  with scale = max |v| (fp32),
+// integer = round-half-even(v / scale * limit), limit = 2^(bits-1) - 1; all in fp32, products and quotients rounded separately.
+template <typename C> __device__ __forceinline__ void fixed_round24(C* v, int bits) {
+  float m = 0.f;
+#pragma unroll
+  for (int k = 0; k < 24; k++) m = fmaxf(m, fabsf((float)v[k]));
+  const float lim = bits == 8 ? 127.f : 32767.f;
+  const float safe = m > 0.f ? m : 1.f;
+#pragma unroll
+  for (int k = 0; k < 24; k++) {
+    const float q = rintf(__fmul_rn(__fdiv_rn((float)v[k], safe), lim));
+    v[k] = m > 0.f ? (C)__fmul_rn(__fdiv_rn(q, lim), m) : (C)0;
+  }
+}
+
 // ------------------------------------------------------------------ K1: Mphi (bidiagonal in s), fused with p-updates
 // mode 0: t = Mphi in                                      (last item of eq. 16)
 // mode 1: p = z + beta p (beta by value), t = Mphi p       (outer iteration, Algorithm 1 line "p = z + beta p")
@@ -340,6 +356,7 @@ template <typename T> struct MphiArgs {
   double beta; const double* beta_dev;   // mode 1: beta by value, or read from device memory when beta_dev != null
   const double* rho; const double* pq;   // inner-CG scalars [it][nblk]
   C diag, off, mf;                  // Mphi = diag*1 + off*(P+ S_minus + P- S_plus), wrap factor -mf
+  int fixed_bits;                   // fp32 storage only: p passes through the 8- / 16-bit fixed-point store of eq. 17 (0 = off)
 };
 
 // true while block `blk` has had rho > 0 and <p,q> > 0 in every iteration 0..it (reading R13: a block that hits
@@ -379,6 +396,7 @@ __global__ void __launch_bounds__(Tile<LS>::NT) k_mphi(const MphiArgs<T> a) {
 #pragma unroll
       for (int k = 0; k < 24; k++) v[k] += beta * p[k];
     }
+    if (sizeof(T) == 4 && a.fixed_bits) fixed_round24(v, a.fixed_bits);
     if (live) store24<T>(a.p, gs, s, LS, v);
     if (sizeof(T) == 2) {  // the operator must act on the stored (rounded) p
 #pragma unroll
@@ -454,7 +472,7 @@ __global__ void k_maxabs(const T* __restrict__ a, long n_sites, int Ls, float* o
 
 // Preconditioner prologue: r = r_in / scale[blk] stored in T;  rho0[blk] += |r|^2 of the STORED values.
 template <typename TIO, typename T>
-__global__ void k_pre_begin(const TIO* __restrict__ rin, T* __restrict__ r, long n_sites, int Ls, const float* scale, double* rho0) {
+__global__ void k_pre_begin(const TIO* __restrict__ rin, T* __restrict__ r, long n_sites, int Ls, const float* scale, double* rho0, int fixed_bits = 0) {
   __shared__ double red[32];
   const SiteThread t = site_thread(n_sites, Ls);
   double part = 0;
@@ -463,10 +481,10 @@ __global__ void k_pre_begin(const TIO* __restrict__ rin, T* __restrict__ r, long
     typename ST<TIO>::C va[24]; typename ST<T>::C vb[24];
     load24<TIO>(rin, t.gsite, t.s, Ls, va);
 #pragma unroll
-    for (int k = 0; k < 24; k++) {
-      vb[k] = round_store((typename ST<T>::C)((double)va[k] * f), (int)sizeof(T));
-      part += (double)vb[k] * (double)vb[k];
-    }
+    for (int k = 0; k < 24; k++) vb[k] = round_store((typename ST<T>::C)((double)va[k] * f), (int)sizeof(T));
+    if (sizeof(T) == 4 && fixed_bits) fixed_round24(vb, fixed_bits);
+#pragma unroll
+    for (int k = 0; k < 24; k++) part += (double)vb[k] * (double)vb[k];
     store24<T>(r, t.gsite, t.s, Ls, vb);
   }
   const double tot = block_sum(part, red, threadIdx.x, blockDim.x);
@@ -479,7 +497,7 @@ __global__ void k_pre_begin(const TIO* __restrict__ rin, T* __restrict__ r, long
 template <typename T, typename TX, typename TIO>
 __global__ void k_inner_update(const T* __restrict__ p, const T* __restrict__ q, T* __restrict__ r, TX* __restrict__ x,
                                TIO* __restrict__ z, long n_sites, int Ls, int it, int nblk, int last,
-                               double* rho, const double* pq, const float* scale) {
+                               double* rho, const double* pq, const float* scale, int fixed_bits = 0) {
   __shared__ double red[32];
   const SiteThread t = site_thread(n_sites, Ls);
   const bool ok = inner_alive(rho, pq, nblk, t.blk, it);
@@ -495,6 +513,7 @@ __global__ void k_inner_update(const T* __restrict__ p, const T* __restrict__ q,
     }
 #pragma unroll
     for (int k = 0; k < 24; k++) vx[k] = (typename ST<TX>::C)((double)vx[k] + alpha * (double)vp[k]);
+    if (sizeof(TX) == 4 && fixed_bits) fixed_round24(vx, fixed_bits);
     if (last) {
       const double f = blk_scale(scale, t.blk);
       typename ST<TIO>::C vz[24];
@@ -507,10 +526,10 @@ __global__ void k_inner_update(const T* __restrict__ p, const T* __restrict__ q,
       load24<T>(q, t.gsite, t.s, Ls, vq);
       load24<T>(r, t.gsite, t.s, Ls, vr);
 #pragma unroll
-      for (int k = 0; k < 24; k++) {
-        vr[k] = round_store((typename ST<T>::C)((double)vr[k] - alpha * (double)vq[k]), (int)sizeof(T));
-        part += (double)vr[k] * (double)vr[k];
-      }
+      for (int k = 0; k < 24; k++) vr[k] = round_store((typename ST<T>::C)((double)vr[k] - alpha * (double)vq[k]), (int)sizeof(T));
+      if (sizeof(T) == 4 && fixed_bits) fixed_round24(vr, fixed_bits);
+#pragma unroll
+      for (int k = 0; k < 24; k++) part += (double)vr[k] * (double)vr[k];
       store24<T>(r, t.gsite, t.s, Ls, vr);
     }
   }
@@ -518,6 +537,51 @@ __global__ void k_inner_update(const T* __restrict__ p, const T* __restrict__ q,
     const double tot = block_sum(part, red, threadIdx.x, blockDim.x);
     if (threadIdx.x == 0 && tot != 0.0) atomicAdd(rho + (long)(it + 1) * nblk + t.blk, tot);
   }
+}
+
+// q <- what a fixed-point store of q returns (eq. 17), and pq[blk] += Re<p, q> of the stored values: the operator output of an inner
+// iteration when the preconditioner's vectors live in fixed-point storage.
+template <typename T>
+__global__ void k_fixed_store_dot(T* __restrict__ q, const T* __restrict__ p, long n_sites, int Ls, int bits, double* pq) {
+  __shared__ double red[32];
+  const SiteThread t = site_thread(n_sites, Ls);
+  double part = 0;
+  if (t.live) {
+    typename ST<T>::C vq[24], vp[24];
+    load24<T>(q, t.gsite, t.s, Ls, vq);
+    load24<T>(p, t.gsite, t.s, Ls, vp);
+    fixed_round24(vq, bits);
+#pragma unroll
+    for (int k = 0; k < 24; k++) part += (double)vp[k] * (double)vq[k];
+    store24<T>(q, t.gsite, t.s, Ls, vq);
+  }
+  const double tot = block_sum(part, red, threadIdx.x, blockDim.x);
+  if (threadIdx.x == 0 && tot != 0.0) atomicAdd(pq + t.blk, tot);
+}
+
+// The storage format itself (eq. 17): ABI vector (fp64, 24 reals per colour-spinor contiguous) <-> 24 signed integers + one fp32 scale per
+// colour-spinor.  One thread per colour-spinor.  INT = int8_t (limit 127) or int16_t (limit 32767).
+template <typename INT>
+__global__ void k_fixed_pack(const double* __restrict__ abi, INT* __restrict__ q, float* __restrict__ scale, long ncs) {
+  const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= ncs) return;
+  const float lim = sizeof(INT) == 1 ? 127.f : 32767.f;
+  float v[24], m = 0.f;
+#pragma unroll
+  for (int k = 0; k < 24; k++) { v[k] = (float)abi[i * 24 + k]; m = fmaxf(m, fabsf(v[k])); }
+  const float safe = m > 0.f ? m : 1.f;
+#pragma unroll
+  for (int k = 0; k < 24; k++) q[i * 24 + k] = m > 0.f ? (INT)__float2int_rn(__fmul_rn(__fdiv_rn(v[k], safe), lim)) : (INT)0;
+  scale[i] = m;
+}
+template <typename INT>
+__global__ void k_fixed_unpack(const INT* __restrict__ q, const float* __restrict__ scale, double* __restrict__ abi, long ncs) {
+  const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= ncs) return;
+  const float lim = sizeof(INT) == 1 ? 127.f : 32767.f;
+  const float m = scale[i];
+#pragma unroll
+  for (int k = 0; k < 24; k++) abi[i * 24 + k] = (double)__fmul_rn(__fdiv_rn((float)q[i * 24 + k], lim), m);
 }
 
 // ------------------------------------------------------------------ reduced-Ls transfer (generic path)

@@ -83,6 +83,7 @@ struct mspcg_ctx {
   GeomDev gfull, gblk;
   TileSet tfull, tblk;
   bool dense_tma = true;         // mspcg_apply_M5inv through dense5d_tma.cuh (MSPCG_M5_TMA=0: the cp.async kernel of transfer_tc.cuh)
+  int fixed_bits = 0;            // 8 / 16: fp32 inner CG vectors pass through the fixed-point store of eq. 17 (mspcg_set_fixed_storage); 0 = off
   int group_blocks = 0;          // Dirichlet blocks per L2-resident group of the preconditioner (0: all blocks at once); MSPCG_GROUP or mspcg_set_block_group
   bool use_tiles = true;         // MSPCG_TILE=0 in the environment selects the per-warp kernel k_hop_mma (A/B measurements)
   int *e_int_to_cb = nullptr, *o_int_to_cb = nullptr;   // FULL list index -> ABI x_cb, even / odd parity
@@ -471,6 +472,9 @@ cudaError_t precond_impl(mspcg_ctx* c, const TIO* r_in_all, TIO* z_out_all, int 
   const int G = (c->group_blocks > 0 && c->group_blocks < nblk) ? c->group_blocks : nblk;
   const size_t io_blk = (size_t)g.nE0 * c->Ls * 24;       // reals of one block's part of an I/O vector (full Ls)
   T *r = (T*)c->in_r, *p = (T*)c->in_p, *q = (T*)c->in_q; TX* x = (TX*)c->in_x;
+  // with fp32 inner storage the CG vectors r, p, q = A p, x can be passed through the 8- / 16-bit fixed-point store of eq. 17
+  // (mspcg_set_fixed_storage): the values are those of fixed-point storage, the bytes in HBM stay fp32 (a numerics mode, not a bandwidth one)
+  const int fb = (sizeof(T) == 4 && !reduced) ? c->fixed_bits : 0;
   for (int g0 = 0; g0 < nblk; g0 += G) {
     const int gn = g0 + G <= nblk ? G : nblk - g0;
     const TIO* r_in = r_in_all + (size_t)g0 * io_blk;
@@ -494,15 +498,21 @@ cudaError_t precond_impl(mspcg_ctx* c, const TIO* r_in_all, TIO* z_out_all, int 
       }
       if (done) {}
       else if (reduced) k_reduce_begin<TIO, T><<<grid_sites(g.nE0, LS, gn), 128, 0, st>>>(r_in, r, g.nE0, c->Ls, LS, c->Tm, scale, rho);
-      else k_pre_begin<TIO, T><<<grid_sites(g.nE0, LS, gn), 128, 0, st>>>(r_in, r, g.nE0, LS, scale, rho); }
+      else k_pre_begin<TIO, T><<<grid_sites(g.nE0, LS, gn), 128, 0, st>>>(r_in, r, g.nE0, LS, scale, rho, fb); }
     c->launches++;
     for (int it = 0; it < k; it++) {
       MphiArgs<T> mp; memset(&mp, 0, sizeof(mp));
-      mp.in = r; mp.p = p; mp.mode = 2; mp.it = it; mp.nblk = nblk; mp.rho = rho; mp.pq = pq;
+      mp.in = r; mp.p = p; mp.mode = 2; mp.it = it; mp.nblk = nblk; mp.rho = rho; mp.pq = pq; mp.fixed_bits = fb;
       if ((e = apply_normal<T, LS>(c, v, mp, p, q, pq + (size_t)it * nblk, st)) != cudaSuccess) return e;
+      if (fb) {   // q = A p goes through the fixed-point store and <p, q> is taken from the stored values
+        if ((e = cudaMemsetAsync(pq + (size_t)it * nblk, 0, sizeof(double) * gn, st)) != cudaSuccess) return e;
+        TimedLaunch tl(c, KIND_BLAS, st);
+        k_fixed_store_dot<T><<<grid_sites(g.nE0, LS, gn), 128, 0, st>>>(q, p, g.nE0, LS, fb, pq + (size_t)it * nblk);
+        c->launches++;
+      }
       { TimedLaunch tl(c, KIND_BLAS, st);
         k_inner_update<T, TX, TIO><<<grid_sites(g.nE0, LS, gn), 128, 0, st>>>(p, q, r, x, z_out, g.nE0, LS, it, nblk, (it == k - 1 && !reduced) ? 1 : 0,
-                                                                              rho, pq, scale); }
+                                                                              rho, pq, scale, fb); }
       c->launches++;
     }
     if (reduced) {
@@ -1466,6 +1476,37 @@ int mspcg_tile_check(mspcg_ctx* ctx, double out_host[8]) {
 int mspcg_set_block_group(mspcg_ctx* ctx, int blocks_per_group) {
   if (!ctx || blocks_per_group < 0) return MSPCG_EINVAL;
   ctx->group_blocks = blocks_per_group;
+  return MSPCG_OK;
+}
+
+int mspcg_set_fixed_storage(mspcg_ctx* ctx, int bits) {
+  if (!ctx) return MSPCG_EINVAL;
+  if (bits != 0 && bits != 8 && bits != 16) return fail(ctx, MSPCG_EINVAL, "mspcg_set_fixed_storage: bits must be 0, 8 or 16");
+  ctx->fixed_bits = bits;
+  return MSPCG_OK;
+}
+
+int mspcg_fixed_pack(mspcg_ctx* ctx, const double* abi_dev, void* q_dev, float* scale_dev, int bits, void* stream) {
+  if (!ctx) return MSPCG_EINVAL;
+  if (!abi_dev || !q_dev || !scale_dev || (bits != 8 && bits != 16)) return fail(ctx, MSPCG_EINVAL, "mspcg_fixed_pack: null pointer or bits not 8 / 16");
+  const long ncs = v5h(ctx, ctx->Ls);
+  const unsigned grid = (unsigned)((ncs + 127) / 128);
+  if (bits == 8) k_fixed_pack<int8_t><<<grid, 128, 0, (cudaStream_t)stream>>>(abi_dev, (int8_t*)q_dev, scale_dev, ncs);
+  else k_fixed_pack<int16_t><<<grid, 128, 0, (cudaStream_t)stream>>>(abi_dev, (int16_t*)q_dev, scale_dev, ncs);
+  ctx->launches++;
+  CUDA_OK(ctx, cudaPeekAtLastError());
+  return MSPCG_OK;
+}
+
+int mspcg_fixed_unpack(mspcg_ctx* ctx, const void* q_dev, const float* scale_dev, double* abi_dev, int bits, void* stream) {
+  if (!ctx) return MSPCG_EINVAL;
+  if (!abi_dev || !q_dev || !scale_dev || (bits != 8 && bits != 16)) return fail(ctx, MSPCG_EINVAL, "mspcg_fixed_unpack: null pointer or bits not 8 / 16");
+  const long ncs = v5h(ctx, ctx->Ls);
+  const unsigned grid = (unsigned)((ncs + 127) / 128);
+  if (bits == 8) k_fixed_unpack<int8_t><<<grid, 128, 0, (cudaStream_t)stream>>>((const int8_t*)q_dev, scale_dev, abi_dev, ncs);
+  else k_fixed_unpack<int16_t><<<grid, 128, 0, (cudaStream_t)stream>>>((const int16_t*)q_dev, scale_dev, abi_dev, ncs);
+  ctx->launches++;
+  CUDA_OK(ctx, cudaPeekAtLastError());
   return MSPCG_OK;
 }
 
