@@ -13,6 +13,7 @@
 #include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <type_traits>
 
 #include "site_math.cuh"
 #include "tile_tables.hpp"
@@ -447,10 +448,12 @@ __global__ void k_convert(const TA* __restrict__ a, TB* __restrict__ b, long n_s
   if (!t.live) return;
   double f = factor;
   if (scale) { const double sc = blk_scale(scale, t.blk); f *= invert ? 1.0 / sc : sc; }
+  typedef typename std::conditional<(sizeof(typename ST<TA>::C) == 8 || sizeof(typename ST<TB>::C) == 8), double, float>::type A;   // no fp64 detour between fp32 / fp16 types (XU pipe)
+  const A fa = (A)f;
   typename ST<TA>::C va[24]; typename ST<TB>::C vb[24];
   load24<TA>(a, t.gsite, t.s, Ls, va);
 #pragma unroll
-  for (int k = 0; k < 24; k++) vb[k] = (typename ST<TB>::C)((double)va[k] * f);
+  for (int k = 0; k < 24; k++) vb[k] = (typename ST<TB>::C)((A)va[k] * fa);
   store24<TB>(b, t.gsite, t.s, Ls, vb);
 }
 
@@ -473,18 +476,22 @@ __global__ void k_maxabs(const T* __restrict__ a, long n_sites, int Ls, float* o
 // Preconditioner prologue: r = r_in / scale[blk] stored in T;  rho0[blk] += |r|^2 of the STORED values.
 template <typename TIO, typename T>
 __global__ void k_pre_begin(const TIO* __restrict__ rin, T* __restrict__ r, long n_sites, int Ls, const float* scale, double* rho0, int fixed_bits = 0) {
+  typedef typename ST<TIO>::C AI;   // arithmetic in the wider of the two register types: fp32 <-> fp64 conversions run on the XU pipe (16 per clock and SM)
+  typedef typename ST<T>::C CT;
   __shared__ double red[32];
   const SiteThread t = site_thread(n_sites, Ls);
   double part = 0;
   if (t.live) {
-    const double f = 1.0 / blk_scale(scale, t.blk);
-    typename ST<TIO>::C va[24]; typename ST<T>::C vb[24];
+    const AI f = (AI)(1.0 / blk_scale(scale, t.blk));
+    AI va[24]; CT vb[24];
     load24<TIO>(rin, t.gsite, t.s, Ls, va);
 #pragma unroll
-    for (int k = 0; k < 24; k++) vb[k] = round_store((typename ST<T>::C)((double)va[k] * f), (int)sizeof(T));
+    for (int k = 0; k < 24; k++) vb[k] = round_store((CT)(va[k] * f), (int)sizeof(T));
     if (sizeof(T) == 4 && fixed_bits) fixed_round24(vb, fixed_bits);
+    CT acc = 0;
 #pragma unroll
-    for (int k = 0; k < 24; k++) part += (double)vb[k] * (double)vb[k];
+    for (int k = 0; k < 24; k++) acc += vb[k] * vb[k];
+    part = (double)acc;
     store24<T>(r, t.gsite, t.s, Ls, vb);
   }
   const double tot = block_sum(part, red, threadIdx.x, blockDim.x);
@@ -498,13 +505,15 @@ template <typename T, typename TX, typename TIO>
 __global__ void k_inner_update(const T* __restrict__ p, const T* __restrict__ q, T* __restrict__ r, TX* __restrict__ x,
                                TIO* __restrict__ z, long n_sites, int Ls, int it, int nblk, int last,
                                double* rho, const double* pq, const float* scale, int fixed_bits = 0) {
+  typedef typename ST<TX>::C A;     // arithmetic type: fp32 unless the storage is fp64 (the scalars stay fp64; per-element fp32 <-> fp64
+  typedef typename ST<T>::C CT;     // conversions would run on the XU pipe and bound the kernel: 55 % busy against DRAM 55 % before)
   __shared__ double red[32];
   const SiteThread t = site_thread(n_sites, Ls);
   const bool ok = inner_alive(rho, pq, nblk, t.blk, it);
-  const double alpha = ok ? rho[(long)it * nblk + t.blk] / pq[(long)it * nblk + t.blk] : 0.0;
+  const A alpha = (A)(ok ? rho[(long)it * nblk + t.blk] / pq[(long)it * nblk + t.blk] : 0.0);
   double part = 0;
   if (t.live) {
-    typename ST<T>::C vp[24]; typename ST<TX>::C vx[24];
+    CT vp[24]; A vx[24];
     load24<T>(p, t.gsite, t.s, Ls, vp);
     if (it > 0) load24<TX>(x, t.gsite, t.s, Ls, vx);
     else {
@@ -512,24 +521,26 @@ __global__ void k_inner_update(const T* __restrict__ p, const T* __restrict__ q,
       for (int k = 0; k < 24; k++) vx[k] = 0;
     }
 #pragma unroll
-    for (int k = 0; k < 24; k++) vx[k] = (typename ST<TX>::C)((double)vx[k] + alpha * (double)vp[k]);
+    for (int k = 0; k < 24; k++) vx[k] = vx[k] + alpha * (A)vp[k];
     if (sizeof(TX) == 4 && fixed_bits) fixed_round24(vx, fixed_bits);
     if (last) {
-      const double f = blk_scale(scale, t.blk);
+      const A f = (A)blk_scale(scale, t.blk);
       typename ST<TIO>::C vz[24];
 #pragma unroll
-      for (int k = 0; k < 24; k++) vz[k] = (typename ST<TIO>::C)((double)vx[k] * f);
+      for (int k = 0; k < 24; k++) vz[k] = (typename ST<TIO>::C)(vx[k] * f);
       store24<TIO>(z, t.gsite, t.s, Ls, vz);
     } else {
       store24<TX>(x, t.gsite, t.s, Ls, vx);
-      typename ST<T>::C vq[24], vr[24];
+      CT vq[24], vr[24];
       load24<T>(q, t.gsite, t.s, Ls, vq);
       load24<T>(r, t.gsite, t.s, Ls, vr);
 #pragma unroll
-      for (int k = 0; k < 24; k++) vr[k] = round_store((typename ST<T>::C)((double)vr[k] - alpha * (double)vq[k]), (int)sizeof(T));
+      for (int k = 0; k < 24; k++) vr[k] = round_store((CT)((A)vr[k] - alpha * (A)vq[k]), (int)sizeof(T));
       if (sizeof(T) == 4 && fixed_bits) fixed_round24(vr, fixed_bits);
+      A acc = 0;
 #pragma unroll
-      for (int k = 0; k < 24; k++) part += (double)vr[k] * (double)vr[k];
+      for (int k = 0; k < 24; k++) acc += (A)vr[k] * (A)vr[k];
+      part = (double)acc;
       store24<T>(r, t.gsite, t.s, Ls, vr);
     }
   }
@@ -729,20 +740,24 @@ __global__ void k_outer_update(const T* __restrict__ p, const T* __restrict__ q,
                                long nchunk, double* __restrict__ sc, int self_z) {
   __shared__ double red[32];
   constexpr int PER = ST<T>::PER;
+  typedef typename ST<T>::C A;      // arithmetic in the register type of the storage (fp32 for fp16 / fp32 storage): no per-element fp64 conversions (XU pipe)
   const double pq = sc[SC_PAP];
   const double alpha = pq > 0.0 ? sc[SC_RZ] / pq : 0.0;
+  const A al = (A)alpha;
   const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
   double part = 0, part2 = 0;
   if (i < nchunk) {
-    typename ST<T>::C vp[PER], vq[PER], vr[PER], vx[PER];
+    A vp[PER], vq[PER], vr[PER], vx[PER];
     ldchunk<T>(p, i, vp); ldchunk<T>(q, i, vq); ldchunk<T>(r, i, vr); ldchunk<T>(x, i, vx);
+    A a1 = 0, a2 = 0;
 #pragma unroll
     for (int k = 0; k < PER; k++) {
-      vx[k] = (typename ST<T>::C)((double)vx[k] + alpha * (double)vp[k]);
-      vr[k] = round_store((typename ST<T>::C)((double)vr[k] - alpha * (double)vq[k]), (int)sizeof(T));
-      part += (double)vr[k] * (double)vr[k];
-      part2 += (double)vr[k] * (double)vq[k];
+      vx[k] = vx[k] + al * vp[k];
+      vr[k] = round_store(vr[k] - al * vq[k], (int)sizeof(T));
+      a1 += vr[k] * vr[k];
+      a2 += vr[k] * vq[k];
     }
+    part = (double)a1; part2 = (double)a2;
     stchunk<T>(x, i, vx); stchunk<T>(r, i, vr);
   }
   const double tot = block_sum(part, red, threadIdx.x, blockDim.x);
@@ -787,8 +802,10 @@ __global__ void k_dot2(const T* __restrict__ a, const T* __restrict__ b, const T
     typename ST<T>::C va[PER], vb[PER], vc[PER];
     ldchunk<T>(a, i, va); ldchunk<T>(b, i, vb);
     if (c) ldchunk<T>(c, i, vc);
+    typename ST<T>::C q0 = 0, q1 = 0;    // one chunk in the register type, then one conversion (no per-element fp64 conversions: XU pipe)
 #pragma unroll
-    for (int k = 0; k < PER; k++) { p0 += (double)va[k] * (double)vb[k]; if (c) p1 += (double)va[k] * (double)vc[k]; }
+    for (int k = 0; k < PER; k++) { q0 += va[k] * vb[k]; if (c) q1 += va[k] * vc[k]; }
+    p0 += (double)q0; p1 += (double)q1;
   }
   const double t0 = block_sum(p0, red, threadIdx.x, blockDim.x);
   __syncthreads();
@@ -805,7 +822,7 @@ __global__ void k_axpby(double a, const T* __restrict__ x, double b, T* __restri
   typename ST<T>::C vx[PER], vy[PER];
   ldchunk<T>(x, i, vx); ldchunk<T>(y, i, vy);
 #pragma unroll
-  for (int k = 0; k < PER; k++) vy[k] = (typename ST<T>::C)(a * (double)vx[k] + b * (double)vy[k]);
+  for (int k = 0; k < PER; k++) vy[k] = (typename ST<T>::C)a * vx[k] + (typename ST<T>::C)b * vy[k];
   stchunk<T>(y, i, vy);
 }
 
