@@ -25,6 +25,9 @@
 
 namespace mspcg {
 
+#ifndef MSPCG_TILE_NSTAGE
+#define MSPCG_TILE_NSTAGE 2   // a third stage fits only for Ls <= 8 (59 KB per stage); measured there: -6 % in kernels 2/4, 0 in 3 and 5
+#endif
 #ifndef MSPCG_TILE_NWC_PLAIN
 #define MSPCG_TILE_NWC_PLAIN 16
 #endif
@@ -33,7 +36,7 @@ namespace mspcg {
 #endif
 template <int LS, int EPI = 0> struct TileCfg {
   enum {
-    TS = TILE_TS, NIN = TILE_NIN, NSTAGE = 2,
+    TS = TILE_TS, NIN = TILE_NIN, NSTAGE = MSPCG_TILE_NSTAGE,
     NWC = MSPCG_TILE_NWC_PLAIN,                     // consumer warps
     PAIR = (MSPCG_TILE_NWC_PLAIN <= 12),            // two sites per warp in one instruction stream (needs 128 registers: at most 12 + 4 warps)
     NWP = MSPCG_TILE_NWP_PLAIN,                     // producer warps
