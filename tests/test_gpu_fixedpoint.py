@@ -79,3 +79,31 @@ def test_preconditioner_with_fixed_point_vectors_matches_oracle():
     with pytest.raises(Exception):
         g.set_fixed_storage(12)
     g.close()
+
+
+def test_fixed_storage_second_geometry_and_scope():
+    """Ls 12, a ragged lattice with an uncut direction; and the mode leaves fp16 / fp64 inner storage alone (include/mspcg.h)."""
+    import torch
+    from paper_2104_05615_b200 import F16, F64
+    dims, Ls, block, k = (4, 6, 4, 4), 12, (2, 6, 2, 2), 3
+    U = synth.gauge_natural_to_abi(synth.random_su3_links(dims, 0.25, 8), dims)
+    ora = Oracle(dims, Ls, MOB["b"], MOB["c"], MOB["M5"], 0.01, block)
+    ora.load_gauge(U, -1)
+    r = synth.gaussian_spinor_abi(dims, Ls, 10)
+    d = torch.as_tensor(r.reshape(-1)).cuda()
+    g = Mspcg(dims, Ls, MOB["b"], MOB["c"], MOB["M5"], 0.01, block)
+    g.configure(F32, F32, 18)
+    g.load_gauge(U, -1)
+    g.set_fixed_storage(16)
+    ref = ora.pack(fx.precond_fixed(ora.precond_obj("PAD"), ora.unpack(r), k, 16))
+    assert rel(g.apply_precond(d, k, F32).cpu().numpy(), ref) <= 2e-4
+    g.close()
+    for inner in (F16, F64):
+        g = Mspcg(dims, Ls, MOB["b"], MOB["c"], MOB["M5"], 0.01, block)
+        g.configure(F64 if inner == F64 else F32, inner, 18)
+        g.load_gauge(U, -1)
+        z0 = g.apply_precond(d, k, F64).cpu().numpy()
+        g.set_fixed_storage(8)
+        # not bitwise: the per-block scalars are summed with atomics; an 8-bit store would show at the 1e-2 level
+        assert rel(g.apply_precond(d, k, F64).cpu().numpy(), z0) <= (1e-12 if inner == F64 else 2e-3)
+        g.close()
